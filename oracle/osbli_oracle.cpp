@@ -1,0 +1,813 @@
+/* osbli_oracle.cpp -- CPU ORACLE (test infrastructure, NOT product code; see osbli_oracle.h).
+ *
+ * A plain, slow, step-by-step restatement of the per-RK-stage residual of PAPER.md
+ * (arXiv 2007.14933) sections 2.1-2.7 and 3.1.3, in the paper's order and notation:
+ *
+ *   O1  point-wise thermodynamics              eq. (6)-(7)
+ *   O2  characteristic flux reconstruction     steps 1-4
+ *       WENO-Z5 / TENO5                        eq. (14)-(26)
+ *   O3  viscous + heat-flux terms              eq. (2)-(5),(28)-(35)
+ *   O4  low-storage RK3                        eq. (36)-(38)
+ *   O5  boundary conditions                    eq. (40)-(46)
+ *
+ * No blocking, fusion or reordering beyond what those passages state.  Build:
+ *   g++ -std=c++17 -O2 -ffp-contract=off -fopenmp -shared -fPIC osbli_oracle.cpp
+ */
+#include "osbli_oracle.h"
+
+#include <cmath>
+#include <cstdlib>
+#include <limits>
+#include <vector>
+
+namespace {
+
+/* ------------------------------------------------------------------ grid bookkeeping ---- */
+struct Grid {
+  int n[3], h[3], N[3];
+  long total;                                  /* one scalar field                          */
+  long idx(int i, int j, int k) const {
+    return ((long)(k + h[2]) * N[1] + (j + h[1])) * N[0] + (i + h[0]);
+  }
+  long stride(int d) const { return d == 0 ? 1 : (d == 1 ? (long)N[0] : (long)N[0] * N[1]); }
+  bool active(int d) const { return n[d] > 1; }
+};
+
+Grid make_grid(const oracle_params *p) {
+  Grid g;
+  for (int d = 0; d < 3; ++d) {
+    g.n[d] = p->n[d];
+    g.h[d] = p->n[d] > 1 ? 3 : 0;
+    g.N[d] = g.n[d] + 2 * g.h[d];
+  }
+  g.total = (long)g.N[0] * g.N[1] * g.N[2];
+  return g;
+}
+
+bool periodic(const oracle_params *p, int d) { return p->bc[d][0] == ORACLE_BC_PERIODIC; }
+
+/* ------------------------------------------------------- O1: point-wise thermodynamics -- */
+struct Prim { double rho, u, v, w, p, a, H, T, mu; };
+
+/* PAPER.md:63-66 eq. (7): p = (gamma-1)(rhoE - rho u_i u_i / 2) = rho T/(gamma M^2),
+ * a = sqrt(gamma p / rho);  PAPER.md:317-318: mu = T^1.5 (1+S)/(T+S), S = SuthT/RefT. */
+Prim prim_of(const oracle_params *p, const double *q) {
+  Prim s;
+  s.rho = q[0];
+  s.u = q[1] / q[0];
+  s.v = q[2] / q[0];
+  s.w = q[3] / q[0];
+  s.p = (p->gamma - 1.0) * (q[4] - 0.5 * s.rho * (s.u * s.u + s.v * s.v + s.w * s.w));
+  s.a = std::sqrt(p->gamma * s.p / s.rho);
+  s.H = (q[4] + s.p) / s.rho;
+  s.T = p->gamma * p->Minf * p->Minf * s.p / s.rho;
+  if (p->visc == ORACLE_VISC_SUTHERLAND) {
+    const double S = p->suth_ratio;
+    s.mu = s.T * std::sqrt(s.T) * (1.0 + S) / (s.T + S);
+  } else {
+    s.mu = 1.0;
+  }
+  return s;
+}
+
+void load_state(const Grid &g, const double *Q, long at, double *q) {
+  for (int c = 0; c < 5; ++c) q[c] = Q[c * g.total + at];
+}
+
+/* ------------------------------------------------------ WENO-Z5 / TENO5 reconstruction -- */
+/* Reconstruct at the interface between c and d; upwind side is a,b,c.
+ * Candidates (eq. 14; coefficients by polynomial exactness, Q3):
+ *   q_R = (2c+5d-e)/6 on {c,d,e};  q_C = (-b+5c+2d)/6 on {b,c,d};  q_L = (2a-7b+11c)/6 on {a,b,c}
+ * ideal weights d_R = 3/10, d_C = 6/10, d_L = 1/10.
+ * Smoothness indicators eq. (17)-(19): beta_0 -> R, beta_1 -> C, beta_2 -> L. */
+double reconstruct(int scheme, double a, double b, double c, double d, double e,
+                   double eps, double ct, double *margin) {
+  const double qR = (2.0 * c + 5.0 * d - e) / 6.0;
+  const double qC = (-b + 5.0 * c + 2.0 * d) / 6.0;
+  const double qL = (2.0 * a - 7.0 * b + 11.0 * c) / 6.0;
+  const double dR = 3.0 / 10.0, dC = 6.0 / 10.0, dL = 1.0 / 10.0;
+
+  const double s0 = c - 2.0 * d + e, t0 = 3.0 * c - 4.0 * d + e;
+  const double s1 = b - 2.0 * c + d, t1 = b - d;
+  const double s2 = a - 2.0 * b + c, t2 = a - 4.0 * b + 3.0 * c;
+  const double bR = 13.0 / 12.0 * (s0 * s0) + 0.25 * (t0 * t0);   /* eq. (17) */
+  const double bC = 13.0 / 12.0 * (s1 * s1) + 0.25 * (t1 * t1);   /* eq. (18) */
+  const double bL = 13.0 / 12.0 * (s2 * s2) + 0.25 * (t2 * t2);   /* eq. (19) */
+  const double tau = std::fabs(bR - bL);                          /* eq. (22) text, eq. (26) */
+
+  if (margin) *margin = std::numeric_limits<double>::infinity();
+
+  if (scheme == ORACLE_WENOZ5) {
+    /* eq. (22): alpha_r = d_r (1 + (tau/(beta_r+eps))^2), omega_r = alpha_r/sum */
+    const double rR = tau / (bR + eps), rC = tau / (bC + eps), rL = tau / (bL + eps);
+    const double aR = dR * (1.0 + rR * rR);
+    const double aC = dC * (1.0 + rC * rC);
+    const double aL = dL * (1.0 + rL * rL);
+    const double sum = aR + aC + aL;
+    const double wR = aR / sum, wC = aC / sum, wL = aL / sum;
+    return wR * qR + wC * qC + wL * qL;                           /* eq. (15) */
+  }
+
+  /* TENO5: eq. (25) gamma_r = (C + tau/(beta_r+eps))^q, C = 1, q = 6 (x^6 = x^2 x^2 x^2);
+   * eq. (24) chi_r = gamma_r / sum; cut-off: delta_r = 0 iff chi_r < C_T; eq. (23). */
+  const double xR = 1.0 + tau / (bR + eps);
+  const double xC = 1.0 + tau / (bC + eps);
+  const double xL = 1.0 + tau / (bL + eps);
+  const double xR2 = xR * xR, xC2 = xC * xC, xL2 = xL * xL;
+  const double gR = xR2 * xR2 * xR2, gC = xC2 * xC2 * xC2, gL = xL2 * xL2 * xL2;
+  const double gsum = gR + gC + gL;
+  const double cR = gR / gsum, cC = gC / gsum, cL = gL / gsum;
+  const double eR = cR < ct ? 0.0 : 1.0;
+  const double eC = cC < ct ? 0.0 : 1.0;
+  const double eL = cL < ct ? 0.0 : 1.0;
+  if (margin) {
+    double m = std::fabs(cR / ct - 1.0);
+    m = std::fmin(m, std::fabs(cC / ct - 1.0));
+    m = std::fmin(m, std::fabs(cL / ct - 1.0));
+    *margin = m;
+  }
+  const double dsum = dR * eR + dC * eC + dL * eL;
+  const double wR = dR * eR / dsum, wC = dC * eC / dsum, wL = dL * eL / dsum;
+  return wR * qR + wC * qC + wL * qL;
+}
+
+/* ---------------------------------------------------------- Roe-averaged eigensystem ---- */
+/* PAPER.md:104-105, steps 2(a)-(b).  Roe average: u_j and H with sqrt(rho) weights, a~ from
+ * H~ (Q11).  Eigenvectors for a general unit normal n without tangent vectors
+ * (Q12); fields ordered 0,1,2 (speed theta), 3 (theta+a), 4 (theta-a). */
+void eigensystem(double gamma, const double *QL, const double *QR, const double *n,
+                 double *L, double *R, double *roe) {
+  const double rL = QL[0], rR = QR[0];
+  const double uL = QL[1] / rL, vL = QL[2] / rL, wL = QL[3] / rL;
+  const double uR = QR[1] / rR, vR = QR[2] / rR, wR = QR[3] / rR;
+  const double pL = (gamma - 1.0) * (QL[4] - 0.5 * rL * (uL * uL + vL * vL + wL * wL));
+  const double pR = (gamma - 1.0) * (QR[4] - 0.5 * rR * (uR * uR + vR * vR + wR * wR));
+  const double HL = (QL[4] + pL) / rL, HR = (QR[4] + pR) / rR;
+  const double sl = std::sqrt(rL), sr = std::sqrt(rR);
+  const double u = (sl * uL + sr * uR) / (sl + sr);
+  const double v = (sl * vL + sr * vR) / (sl + sr);
+  const double w = (sl * wL + sr * wR) / (sl + sr);
+  const double H = (sl * HL + sr * HR) / (sl + sr);
+  const double q2 = u * u + v * v + w * w;
+  const double a = std::sqrt((gamma - 1.0) * (H - 0.5 * q2));
+  const double nx = n[0], ny = n[1], nz = n[2];
+  const double th = nx * u + ny * v + nz * w;
+  const double b1 = (gamma - 1.0) / (a * a);
+  const double b2 = 0.5 * b1 * q2;
+  if (roe) { roe[0] = u; roe[1] = v; roe[2] = w; roe[3] = H; roe[4] = a; }
+
+  /* right eigenvectors r_k = column k of R (R[row*5 + k]) */
+  const double r0[5] = {nx, u * nx, v * nx + nz, w * nx - ny, 0.5 * q2 * nx + v * nz - w * ny};
+  const double r1[5] = {ny, u * ny - nz, v * ny, w * ny + nx, 0.5 * q2 * ny + w * nx - u * nz};
+  const double r2[5] = {nz, u * nz + ny, v * nz - nx, w * nz, 0.5 * q2 * nz + u * ny - v * nx};
+  const double r3[5] = {1.0, u + a * nx, v + a * ny, w + a * nz, H + a * th};
+  const double r4[5] = {1.0, u - a * nx, v - a * ny, w - a * nz, H - a * th};
+  for (int r = 0; r < 5; ++r) {
+    R[r * 5 + 0] = r0[r]; R[r * 5 + 1] = r1[r]; R[r * 5 + 2] = r2[r];
+    R[r * 5 + 3] = r3[r]; R[r * 5 + 4] = r4[r];
+  }
+  /* left eigenvectors l_k = row k of L */
+  const double l0[5] = {nx * (1.0 - b2) - (v * nz - w * ny), nx * b1 * u, nx * b1 * v + nz, nx * b1 * w - ny, -nx * b1};
+  const double l1[5] = {ny * (1.0 - b2) - (w * nx - u * nz), ny * b1 * u - nz, ny * b1 * v, ny * b1 * w + nx, -ny * b1};
+  const double l2[5] = {nz * (1.0 - b2) - (u * ny - v * nx), nz * b1 * u + ny, nz * b1 * v - nx, nz * b1 * w, -nz * b1};
+  const double l3[5] = {0.5 * (b2 - th / a), 0.5 * (-b1 * u + nx / a), 0.5 * (-b1 * v + ny / a), 0.5 * (-b1 * w + nz / a), 0.5 * b1};
+  const double l4[5] = {0.5 * (b2 + th / a), 0.5 * (-b1 * u - nx / a), 0.5 * (-b1 * v - ny / a), 0.5 * (-b1 * w - nz / a), 0.5 * b1};
+  for (int c = 0; c < 5; ++c) {
+    L[0 * 5 + c] = l0[c]; L[1 * 5 + c] = l1[c]; L[2 * 5 + c] = l2[c];
+    L[3 * 5 + c] = l3[c]; L[4 * 5 + c] = l4[c];
+  }
+}
+
+/* ------------------------------------------- O2: interface flux along one direction ----- */
+/* Area-weighted normal K_m of step 1 (Q13, Q24): uniform K = e_d; curvilinear
+ * K = J (D_d0, D_d1, D_d2) with point-wise metrics. */
+void normal_at(const oracle_params *p, int dir, long at, double *K) {
+  if (!p->curvilinear) {
+    K[0] = K[1] = K[2] = 0.0;
+    K[dir] = 1.0;
+  } else {
+    const double J = p->detJ[at];
+    for (int c = 0; c < 3; ++c) K[c] = J * p->D[dir][c][at];
+  }
+}
+
+/* f^_{i+1/2} between node `at` and `at + stride(dir)`; PAPER.md:100-111 steps 1-2. */
+void interface_flux(const oracle_params *p, const Grid &g, const double *Q, int dir, long at,
+                    double *fhat, double *margin) {
+  const long s = g.stride(dir);
+  double U[6][5], F[6][5], lam0[6], lamp[6], lamm[6], K[6][3];
+
+  /* step 1: flux f(U_m), solution vector U_m and wave speeds at the stencil points i-2..i+3 */
+  for (int m = 0; m < 6; ++m) {
+    const long pt = at + (long)(m - 2) * s;
+    load_state(g, Q, pt, U[m]);
+    const Prim w = prim_of(p, U[m]);
+    normal_at(p, dir, pt, K[m]);
+    const double th = K[m][0] * w.u + K[m][1] * w.v + K[m][2] * w.w;
+    const double Kn = std::sqrt(K[m][0] * K[m][0] + K[m][1] * K[m][1] + K[m][2] * K[m][2]);
+    F[m][0] = w.rho * th;
+    F[m][1] = U[m][1] * th + w.p * K[m][0];
+    F[m][2] = U[m][2] * th + w.p * K[m][1];
+    F[m][3] = U[m][3] * th + w.p * K[m][2];
+    F[m][4] = (U[m][4] + w.p) * th;
+    lam0[m] = th;
+    lamp[m] = th + w.a * Kn;
+    lamm[m] = th - w.a * Kn;
+  }
+
+  /* step 2(a)-(b): Roe average of nodes i, i+1 and its eigensystem; interface normal from
+   * the averaged K (uniform: e_d). */
+  double nhat[3];
+  {
+    const double kx = 0.5 * (K[2][0] + K[3][0]);
+    const double ky = 0.5 * (K[2][1] + K[3][1]);
+    const double kz = 0.5 * (K[2][2] + K[3][2]);
+    const double kn = std::sqrt(kx * kx + ky * ky + kz * kz);
+    nhat[0] = kx / kn; nhat[1] = ky / kn; nhat[2] = kz / kn;
+  }
+  double L[25], R[25];
+  eigensystem(p->gamma, U[2], U[3], nhat, L, R, nullptr);
+
+  for (int c = 0; c < 5; ++c) fhat[c] = 0.0;
+  double mmin = std::numeric_limits<double>::infinity();
+
+  for (int k = 0; k < 5; ++k) {
+    /* step 2(c): V_k,m = l_k . U_m, G_k,m = l_k . f_m */
+    double V[6], G[6];
+    for (int m = 0; m < 6; ++m) {
+      double sv = 0.0, sg = 0.0;
+      for (int c = 0; c < 5; ++c) {
+        sv += L[k * 5 + c] * U[m][c];
+        sg += L[k * 5 + c] * F[m][c];
+      }
+      V[m] = sv;
+      G[m] = sg;
+    }
+    /* step 2(d): alpha_k = max over the 6 stencil points of |lambda_k| (Q10) */
+    const double *lam = (k < 3) ? lam0 : (k == 3 ? lamp : lamm);
+    double alpha = 0.0;
+    for (int m = 0; m < 6; ++m) alpha = std::fmax(alpha, std::fabs(lam[m]));
+    double gp[6], gm[6];
+    for (int m = 0; m < 6; ++m) {
+      gp[m] = 0.5 * (G[m] + alpha * V[m]);          /* eq. (13) */
+      gm[m] = 0.5 * (G[m] - alpha * V[m]);
+    }
+    /* step 2(e): g+ from the left-biased stencil, g- from its mirror image (Q4) */
+    double m1, m2;
+    const double hp = reconstruct(p->scheme, gp[0], gp[1], gp[2], gp[3], gp[4], p->eps, p->teno_ct, &m1);
+    const double hm = reconstruct(p->scheme, gm[5], gm[4], gm[3], gm[2], gm[1], p->eps, p->teno_ct, &m2);
+    mmin = std::fmin(mmin, std::fmin(m1, m2));
+    /* step 2(f): back to physical space, f^ += (g^+ + g^-) r_k */
+    const double gk = hp + hm;
+    for (int c = 0; c < 5; ++c) fhat[c] += gk * R[c * 5 + k];
+  }
+  if (margin) *margin = mmin;
+}
+
+/* ----------------------------------------------- central differences, eq. (28)-(35) ----- */
+/* Coefficients (times 12 delta) of the first derivative at node i of a line of n nodes.
+ * Interior: eq. (28) with the sign corrected (Q1): (f_-2 - 8 f_-1 + 8 f_+1 - f_+2).
+ * Non-periodic ends: eq. (30)-(33).  Returns the offset of the first stencil node. */
+int d1_coeffs(int n, int i, bool per, double *c) {
+  if (!per && i == 0)      { c[0] = -25; c[1] = 48;  c[2] = -36; c[3] = 16;  c[4] = -3; return 0; }   /* (30) */
+  if (!per && i == 1)      { c[0] = -3;  c[1] = -10; c[2] = 18;  c[3] = -6;  c[4] = 1;  return -1; }  /* (31) */
+  if (!per && i == n - 2)  { c[0] = -1;  c[1] = 6;   c[2] = -18; c[3] = 10;  c[4] = 3;  return -3; }  /* (32) */
+  if (!per && i == n - 1)  { c[0] = 3;   c[1] = -16; c[2] = 36;  c[3] = -48; c[4] = 25; return -4; }  /* (33) */
+  c[0] = 1; c[1] = -8; c[2] = 0; c[3] = 8; c[4] = -1;                                                 /* (28) */
+  return -2;
+}
+/* Second derivative: interior eq. (29); ends eq. (34)-(35) and their mirror images. */
+int d2_coeffs(int n, int i, bool per, double *c) {
+  if (!per && i == 0)      { c[0] = 35; c[1] = -104; c[2] = 114; c[3] = -56;  c[4] = 11; return 0; }  /* (34) */
+  if (!per && i == 1)      { c[0] = 11; c[1] = -20;  c[2] = 6;   c[3] = 4;    c[4] = -1; return -1; } /* (35) */
+  if (!per && i == n - 2)  { c[0] = -1; c[1] = 4;    c[2] = 6;   c[3] = -20;  c[4] = 11; return -3; }
+  if (!per && i == n - 1)  { c[0] = 11; c[1] = -56;  c[2] = 114; c[3] = -104; c[4] = 35; return -4; }
+  c[0] = -1; c[1] = 16; c[2] = -30; c[3] = 16; c[4] = -1;                                             /* (29) */
+  return -2;
+}
+
+double d1_line(const double *f, long s, int n, int i, bool per, double delta) {
+  double c[5];
+  const int o = d1_coeffs(n, i, per, c);
+  double acc = 0.0;
+  for (int m = 0; m < 5; ++m) acc += c[m] * f[(long)(i + o + m) * s];
+  return acc / (12.0 * delta);
+}
+double d2_line(const double *f, long s, int n, int i, bool per, double delta) {
+  double c[5];
+  const int o = d2_coeffs(n, i, per, c);
+  double acc = 0.0;
+  for (int m = 0; m < 5; ++m) acc += c[m] * f[(long)(i + o + m) * s];
+  return acc / (12.0 * delta * delta);
+}
+
+/* ------------------------------------------------ O3: viscous and heat-flux terms ------- */
+/* Source of primitive values u,v,w,T,mu: either whole-field arrays (full residual) or
+ * computed on the fly from Q (sampled residual).  Same function, same bits. */
+struct PrimSource {
+  const oracle_params *p;
+  const Grid *g;
+  const double *Q;
+  const double *fields;   /* 5 fields u,v,w,T,mu in oracle layout, or NULL */
+  double get(int f, long at) const {
+    if (fields) return fields[f * g->total + at];
+    double q[5];
+    load_state(*g, Q, at, q);
+    const Prim s = prim_of(p, q);
+    switch (f) { case 0: return s.u; case 1: return s.v; case 2: return s.w; case 3: return s.T; default: return s.mu; }
+  }
+};
+
+struct NodeIdx { int c[3]; };
+
+/* delta_k f at a node (first difference along xi_k) */
+double dk(const PrimSource &ps, int f, int k, NodeIdx nd, long at) {
+  const Grid &g = *ps.g;
+  if (!g.active(k)) return 0.0;
+  const bool per = periodic(ps.p, k);
+  const double delta = ps.p->curvilinear ? 1.0 : ps.p->delta[k];
+  double c[5];
+  const int o = d1_coeffs(g.n[k], nd.c[k], per, c);
+  const long s = g.stride(k);
+  double acc = 0.0;
+  for (int m = 0; m < 5; ++m) acc += c[m] * ps.get(f, at + (long)(o + m) * s);
+  return acc / (12.0 * delta);
+}
+/* delta_kk f */
+double dkk(const PrimSource &ps, int f, int k, NodeIdx nd, long at) {
+  const Grid &g = *ps.g;
+  if (!g.active(k)) return 0.0;
+  const bool per = periodic(ps.p, k);
+  const double delta = ps.p->curvilinear ? 1.0 : ps.p->delta[k];
+  double c[5];
+  const int o = d2_coeffs(g.n[k], nd.c[k], per, c);
+  const long s = g.stride(k);
+  double acc = 0.0;
+  for (int m = 0; m < 5; ++m) acc += c[m] * ps.get(f, at + (long)(o + m) * s);
+  return acc / (12.0 * delta * delta);
+}
+/* delta_kl f := delta_k (delta_l f), k < l, fixed order of composition */
+double dkl(const PrimSource &ps, int f, int k, int l, NodeIdx nd, long at) {
+  const Grid &g = *ps.g;
+  if (!g.active(k) || !g.active(l)) return 0.0;
+  const bool per = periodic(ps.p, k);
+  const double delta = ps.p->curvilinear ? 1.0 : ps.p->delta[k];
+  double c[5];
+  const int o = d1_coeffs(g.n[k], nd.c[k], per, c);
+  const long s = g.stride(k);
+  double acc = 0.0;
+  for (int m = 0; m < 5; ++m) {
+    if (c[m] == 0.0) continue;
+    NodeIdx sh = nd;
+    sh.c[k] += o + m;
+    acc += c[m] * dk(ps, f, l, sh, at + (long)(o + m) * s);
+  }
+  return acc / (12.0 * delta);
+}
+
+const int IJ[3][3] = {{0, 1, 2}, {1, 3, 4}, {2, 4, 5}};   /* (i,j) -> index into xx,xy,xz,yy,yz,zz */
+
+/* Adds the viscous + heat-flux contribution at one node to r[5].  PAPER.md:49-57 eq. (2)-(5)
+ * expanded by the product rule (Q21); metric chain rule PAPER.md:228 (Q25). */
+void viscous_at(const PrimSource &ps, NodeIdx nd, long at, double *r) {
+  const oracle_params *p = ps.p;
+  /* computational differences of u,v,w,T (f = 0..3) and mu (f = 4) */
+  double c1[5][3], c2[4][3][3];
+  for (int f = 0; f < 5; ++f)
+    for (int k = 0; k < 3; ++k) c1[f][k] = (f == 4 && p->visc != ORACLE_VISC_SUTHERLAND) ? 0.0 : dk(ps, f, k, nd, at);
+  for (int f = 0; f < 4; ++f)
+    for (int k = 0; k < 3; ++k)
+      for (int l = k; l < 3; ++l) {
+        const double v = (k == l) ? dkk(ps, f, k, nd, at) : dkl(ps, f, k, l, nd, at);
+        c2[f][k][l] = v;
+        c2[f][l][k] = v;
+      }
+  /* physical derivatives: uniform d_j f = delta_j f; curvilinear d_j f = sum_k D_kj delta_k f,
+   * d_i d_j f = sum_k sum_l D_ki D_lj delta_kl f + sum_l E_l,ij delta_l f */
+  double g1[5][3], g2[4][3][3];
+  if (!p->curvilinear) {
+    for (int f = 0; f < 5; ++f) for (int j = 0; j < 3; ++j) g1[f][j] = c1[f][j];
+    for (int f = 0; f < 4; ++f) for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) g2[f][i][j] = c2[f][i][j];
+  } else {
+    double D[3][3], E[3][6];
+    for (int k = 0; k < 3; ++k) {
+      for (int j = 0; j < 3; ++j) D[k][j] = p->D[k][j][at];
+      for (int m = 0; m < 6; ++m) E[k][m] = p->E[k][m][at];
+    }
+    for (int f = 0; f < 5; ++f)
+      for (int j = 0; j < 3; ++j) {
+        double acc = 0.0;
+        for (int k = 0; k < 3; ++k) acc += D[k][j] * c1[f][k];
+        g1[f][j] = acc;
+      }
+    for (int f = 0; f < 4; ++f)
+      for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) {
+          double acc = 0.0;
+          for (int k = 0; k < 3; ++k)
+            for (int l = 0; l < 3; ++l) acc += D[k][i] * D[l][j] * c2[f][k][l];
+          for (int l = 0; l < 3; ++l) acc += E[l][IJ[i][j]] * c1[f][l];
+          g2[f][i][j] = acc;
+        }
+  }
+  const double vel[3] = {ps.get(0, at), ps.get(1, at), ps.get(2, at)};
+  const double mu = ps.get(4, at);
+  const double div = g1[0][0] + g1[1][1] + g1[2][2];
+  const double *dmu = g1[4];
+  const double *dT = g1[3];
+
+  /* M_i = Re * d_j tau_ij */
+  double M[3];
+  for (int i = 0; i < 3; ++i) {
+    const double lap = g2[i][0][0] + g2[i][1][1] + g2[i][2][2];
+    const double gdiv = g2[0][i][0] + g2[1][i][1] + g2[2][i][2];        /* d_i (d_k u_k) */
+    double cross = 0.0;
+    for (int j = 0; j < 3; ++j) cross += dmu[j] * (g1[i][j] + g1[j][i]);
+    M[i] = mu * (lap + gdiv / 3.0) + cross - 2.0 / 3.0 * dmu[i] * div;
+  }
+  /* tau_ij d_j u_i, eq. (5) */
+  double phi = 0.0;
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) {
+      const double tau = mu / p->Re * (g1[i][j] + g1[j][i] - (i == j ? 2.0 / 3.0 * div : 0.0));
+      phi += tau * g1[i][j];
+    }
+  /* -d_j q_j, eq. (4) */
+  const double cq = 1.0 / ((p->gamma - 1.0) * p->Minf * p->Minf * p->Pr * p->Re);
+  const double lapT = g2[3][0][0] + g2[3][1][1] + g2[3][2][2];
+  const double heat = cq * (mu * lapT + (dmu[0] * dT[0] + dmu[1] * dT[1] + dmu[2] * dT[2]));
+
+  r[1] += M[0] / p->Re;
+  r[2] += M[1] / p->Re;
+  r[3] += M[2] / p->Re;
+  r[4] += (vel[0] * M[0] + vel[1] * M[1] + vel[2] * M[2]) / p->Re + phi + heat;
+}
+
+void fill_prim_fields(const oracle_params *p, const Grid &g, const double *Q, double *fields) {
+#pragma omp parallel for num_threads(p->nthreads) schedule(static)
+  for (long at = 0; at < g.total; ++at) {
+    double q[5];
+    load_state(g, Q, at, q);
+    const Prim s = prim_of(p, q);
+    fields[0 * g.total + at] = s.u;
+    fields[1 * g.total + at] = s.v;
+    fields[2 * g.total + at] = s.w;
+    fields[3 * g.total + at] = s.T;
+    fields[4 * g.total + at] = s.mu;
+  }
+}
+
+/* ------------------------------------------------- metric terms ---------- */
+/* "The metric terms are evaluated by the same central interior and boundary schemes ...
+ * computed once at the start of the simulation."  Given node coordinates x_j(xi) on the
+ * halo-extended grid (halos hold the periodic continuation where the direction is periodic;
+ * they are not read otherwise), compute A_jk = d x_j/d xi_k with delta_k (eq. 28, 30-33, unit
+ * computational spacing), J = det A, D = A^-1 (D_kj = d xi_k/d x_j), and
+ * E_l,ij = d_i(D_lj) = sum_k D_ki delta_k(D_lj) for i <= j (Q25).  Halo values of
+ * D, J, E: periodic wrap, else copy of the boundary plane (Q25).  An inactive
+ * direction k has A_jk = delta[k] if j == k else 0. */
+void fill_field_halo(const oracle_params *p, const Grid &g, double *f) {
+  for (int d = 0; d < 3; ++d) {
+    if (!g.active(d)) continue;
+    int lo[3], hi[3];
+    for (int e = 0; e < 3; ++e) {
+      if (e < d) { lo[e] = -g.h[e]; hi[e] = g.n[e] + g.h[e]; }
+      else       { lo[e] = 0;       hi[e] = g.n[e]; }
+    }
+    const long s = g.stride(d);
+    const int n = g.n[d];
+    const int e1 = (d + 1) % 3, e2 = (d + 2) % 3;
+    for (int a = lo[e2]; a < hi[e2]; ++a)
+      for (int b = lo[e1]; b < hi[e1]; ++b) {
+        int ijk[3];
+        ijk[d] = 0; ijk[e1] = b; ijk[e2] = a;
+        const long base = g.idx(ijk[0], ijk[1], ijk[2]);
+        for (int m = 1; m <= 3; ++m) {
+          if (periodic(p, d)) {
+            f[base - (long)m * s] = f[base + (long)(n - m) * s];
+            f[base + (long)(n - 1 + m) * s] = f[base + (long)(m - 1) * s];
+          } else {
+            f[base - (long)m * s] = f[base];
+            f[base + (long)(n - 1 + m) * s] = f[base + (long)(n - 1) * s];
+          }
+        }
+      }
+  }
+}
+
+void metrics_from_coords(const oracle_params *p, const Grid &g, const double *X,
+                         double *const *D, double *detJ, double *const *E) {
+  const int nt = p->nthreads;
+#pragma omp parallel for num_threads(nt) schedule(static)
+  for (int k = 0; k < g.n[2]; ++k)
+    for (int j = 0; j < g.n[1]; ++j)
+      for (int i = 0; i < g.n[0]; ++i) {
+        const long at = g.idx(i, j, k);
+        const int nd[3] = {i, j, k};
+        double A[3][3];
+        for (int c = 0; c < 3; ++c)
+          for (int d = 0; d < 3; ++d) {
+            if (!g.active(d)) { A[c][d] = (c == d) ? p->delta[d] : 0.0; continue; }
+            /* base pointer of the line through this node along d, node index nd[d] */
+            const double *line = X + c * g.total + at - (long)nd[d] * g.stride(d);
+            A[c][d] = d1_line(line, g.stride(d), g.n[d], nd[d], periodic(p, d), 1.0);
+          }
+        const double det = A[0][0] * (A[1][1] * A[2][2] - A[1][2] * A[2][1])
+                         - A[0][1] * (A[1][0] * A[2][2] - A[1][2] * A[2][0])
+                         + A[0][2] * (A[1][0] * A[2][1] - A[1][1] * A[2][0]);
+        detJ[at] = det;
+        /* inverse by cofactors: D[k][j] = cof(A)[j][k] / det */
+        D[0 * 3 + 0][at] = (A[1][1] * A[2][2] - A[1][2] * A[2][1]) / det;
+        D[0 * 3 + 1][at] = (A[0][2] * A[2][1] - A[0][1] * A[2][2]) / det;
+        D[0 * 3 + 2][at] = (A[0][1] * A[1][2] - A[0][2] * A[1][1]) / det;
+        D[1 * 3 + 0][at] = (A[1][2] * A[2][0] - A[1][0] * A[2][2]) / det;
+        D[1 * 3 + 1][at] = (A[0][0] * A[2][2] - A[0][2] * A[2][0]) / det;
+        D[1 * 3 + 2][at] = (A[0][2] * A[1][0] - A[0][0] * A[1][2]) / det;
+        D[2 * 3 + 0][at] = (A[1][0] * A[2][1] - A[1][1] * A[2][0]) / det;
+        D[2 * 3 + 1][at] = (A[0][1] * A[2][0] - A[0][0] * A[2][1]) / det;
+        D[2 * 3 + 2][at] = (A[0][0] * A[1][1] - A[0][1] * A[1][0]) / det;
+      }
+  for (int m = 0; m < 9; ++m) fill_field_halo(p, g, D[m]);
+  fill_field_halo(p, g, detJ);
+#pragma omp parallel for num_threads(nt) schedule(static)
+  for (int k = 0; k < g.n[2]; ++k)
+    for (int j = 0; j < g.n[1]; ++j)
+      for (int i = 0; i < g.n[0]; ++i) {
+        const long at = g.idx(i, j, k);
+        const int nd[3] = {i, j, k};
+        for (int l = 0; l < 3; ++l)
+          for (int a = 0; a < 3; ++a)
+            for (int b = a; b < 3; ++b) {
+              double acc = 0.0;                      /* d_a (D_lb) = sum_k D_ka delta_k (D_lb) */
+              for (int d = 0; d < 3; ++d) {
+                if (!g.active(d)) continue;
+                const double *line = D[l * 3 + b] + at - (long)nd[d] * g.stride(d);
+                acc += D[d * 3 + a][at] * d1_line(line, g.stride(d), g.n[d], nd[d], periodic(p, d), 1.0);
+              }
+              E[l * 6 + IJ[a][b]][at] = acc;
+            }
+      }
+  for (int m = 0; m < 18; ++m) fill_field_halo(p, g, E[m]);
+}
+
+/* Divisor of eq. (10): Delta_d (uniform) or J_i (curvilinear, unit computational spacing). */
+double flux_divisor(const oracle_params *p, int dir, long at) {
+  return p->curvilinear ? p->detJ[at] : p->delta[dir];
+}
+
+int validate(const oracle_params *p) {
+  for (int d = 0; d < 3; ++d) {
+    if (p->n[d] < 1) return 1;
+    if (p->n[d] > 1 && p->n[d] < 5) return 1;
+    if ((p->bc[d][0] == ORACLE_BC_PERIODIC) != (p->bc[d][1] == ORACLE_BC_PERIODIC)) return 1;
+  }
+  if (p->nthreads < 1) return 1;
+  return 0;
+}
+
+/* -------------------------------------------------------------- O5: boundary fill ------- */
+void bc_direction(const oracle_params *p, const Grid &g, double *Q, int d) {
+  if (!g.active(d)) return;
+  /* transverse ranges: directions below d are taken over their halo-extended range, the
+   * ones above d over the interior only (they are filled afterwards) */
+  int lo[3], hi[3];
+  for (int e = 0; e < 3; ++e) {
+    if (e < d) { lo[e] = -g.h[e]; hi[e] = g.n[e] + g.h[e]; }
+    else       { lo[e] = 0;       hi[e] = g.n[e]; }
+  }
+  const long s = g.stride(d);
+  const int n = g.n[d];
+  const int e1 = (d + 1) % 3, e2 = (d + 2) % 3;
+  const double gam = p->gamma, M2 = p->Minf * p->Minf;
+  for (int a = lo[e2]; a < hi[e2]; ++a)
+    for (int b = lo[e1]; b < hi[e1]; ++b) {
+      int ijk[3];
+      ijk[d] = 0; ijk[e1] = b; ijk[e2] = a;
+      const long base = g.idx(ijk[0], ijk[1], ijk[2]);      /* node 0 of this line */
+      for (int side = 0; side < 2; ++side) {
+        const int type = p->bc[d][side];
+        /* wall: node index of the boundary plane; inw: +1 into the domain */
+        const long wall = base + (side == 0 ? 0 : (long)(n - 1) * s);
+        const long inw = side == 0 ? s : -s;
+        if (type == ORACLE_BC_PERIODIC) {
+          for (int m = 1; m <= 3; ++m)
+            for (int c = 0; c < 5; ++c) {
+              double *q = Q + c * g.total;
+              if (side == 0) q[base - (long)m * s] = q[base + (long)(n - m) * s];
+              else           q[base + (long)(n - 1 + m) * s] = q[base + (long)(m - 1) * s];
+            }
+        } else if (type == ORACLE_BC_EXTRAP0) {
+          for (int m = 1; m <= 3; ++m)
+            for (int c = 0; c < 5; ++c) Q[c * g.total + wall - (long)m * inw] = Q[c * g.total + wall];
+        } else if (type == ORACLE_BC_DIRICHLET) {
+          for (int m = 0; m <= 3; ++m)
+            for (int c = 0; c < 5; ++c)
+              Q[c * g.total + wall - (long)m * inw] = p->dirichlet[c * g.total + wall - (long)m * inw];
+        } else if (type == ORACLE_BC_WALL_ISOTHERMAL) {
+          const double Tw = p->wall_T[d][side];
+          /* eq. (40)-(41): no-slip on the boundary plane, wall energy from T_w; rho_w floats */
+          const double rw = Q[wall];
+          Q[1 * g.total + wall] = 0.0;
+          Q[2 * g.total + wall] = 0.0;
+          Q[3 * g.total + wall] = 0.0;
+          const double Ew = rw * Tw / (M2 * gam * (gam - 1.0));
+          Q[4 * g.total + wall] = Ew;
+          const double pw = (gam - 1.0) * Ew;
+          /* T_1: temperature of the first interior node */
+          double q1[5];
+          load_state(g, Q, wall + inw, q1);
+          const double T1 = prim_of(p, q1).T;
+          for (int m = 1; m <= 3; ++m) {
+            const double Tm = (m + 1) * Tw - m * T1;                       /* eq. (42) */
+            const double rm = M2 * gam * pw / Tm;                          /* eq. (43) */
+            double qi[5];
+            load_state(g, Q, wall + (long)m * inw, qi);
+            const double ui = qi[1] / qi[0], vi = qi[2] / qi[0], wi = qi[3] / qi[0];
+            const long at = wall - (long)m * inw;
+            Q[0 * g.total + at] = rm;
+            Q[1 * g.total + at] = -rm * ui;                                /* eq. (44) */
+            Q[2 * g.total + at] = -rm * vi;                                /* eq. (45) */
+            Q[3 * g.total + at] = -rm * wi;                                /* eq. (46) */
+            Q[4 * g.total + at] = pw / (gam - 1.0) + 0.5 * rm * (ui * ui + vi * vi + wi * wi);
+          }
+        }
+      }
+    }
+}
+
+void rhs_full(const oracle_params *p, const Grid &g, const double *Q, double *R, int parts, double *margin) {
+  const int nt = p->nthreads;
+  /* R starts at 0 on interior nodes */
+#pragma omp parallel for num_threads(nt) schedule(static)
+  for (int k = 0; k < g.n[2]; ++k)
+    for (int j = 0; j < g.n[1]; ++j)
+      for (int i = 0; i < g.n[0]; ++i) {
+        const long at = g.idx(i, j, k);
+        for (int c = 0; c < 5; ++c) R[c * g.total + at] = 0.0;
+        if (margin) margin[at] = std::numeric_limits<double>::infinity();
+      }
+
+  if (parts & ORACLE_PART_INVISCID) {
+    for (int d = 0; d < 3; ++d) {
+      if (!g.active(d)) continue;                      /* step 4: repeat for all dimensions */
+      const int e1 = (d + 1) % 3, e2 = (d + 2) % 3;
+      const int n = g.n[d];
+      const long s = g.stride(d);
+#pragma omp parallel for num_threads(nt) schedule(static) collapse(2)
+      for (int a = 0; a < g.n[e2]; ++a)
+        for (int b = 0; b < g.n[e1]; ++b) {
+          int ijk[3];
+          ijk[d] = 0; ijk[e1] = b; ijk[e2] = a;
+          const long base = g.idx(ijk[0], ijk[1], ijk[2]);
+          /* step 2: every half node of this line, -1/2 ... n-1/2 */
+          std::vector<double> fh((size_t)(n + 1) * 5), mg((size_t)n + 1);
+          for (int q = 0; q <= n; ++q)
+            interface_flux(p, g, Q, d, base + (long)(q - 1) * s, &fh[(size_t)q * 5], &mg[q]);
+          /* step 3: eq. (10) */
+          for (int i = 0; i < n; ++i) {
+            const long at = base + (long)i * s;
+            const double div = flux_divisor(p, d, at);
+            for (int c = 0; c < 5; ++c)
+              R[c * g.total + at] -= (fh[(size_t)(i + 1) * 5 + c] - fh[(size_t)i * 5 + c]) / div;
+            if (margin) margin[at] = std::fmin(margin[at], std::fmin(mg[i], mg[i + 1]));
+          }
+        }
+    }
+  }
+
+  if ((parts & ORACLE_PART_VISCOUS) && p->visc != ORACLE_VISC_NONE) {
+    std::vector<double> fields((size_t)5 * g.total);
+    fill_prim_fields(p, g, Q, fields.data());
+    PrimSource ps{p, &g, Q, fields.data()};
+#pragma omp parallel for num_threads(nt) schedule(static)
+    for (int k = 0; k < g.n[2]; ++k)
+      for (int j = 0; j < g.n[1]; ++j)
+        for (int i = 0; i < g.n[0]; ++i) {
+          const long at = g.idx(i, j, k);
+          double r[5] = {0, 0, 0, 0, 0};
+          viscous_at(ps, NodeIdx{{i, j, k}}, at, r);
+          for (int c = 1; c < 5; ++c) R[c * g.total + at] += r[c];
+        }
+  }
+}
+
+}  // namespace
+
+/* ======================================================================== C entry points */
+extern "C" {
+
+double oracle_reconstruct(int32_t scheme, double a, double b, double c, double d, double e,
+                          double eps, double teno_ct, double *margin) {
+  return reconstruct(scheme, a, b, c, d, e, eps, teno_ct, margin);
+}
+
+void oracle_eigensystem(double gamma, const double *QL, const double *QR, const double *nhat,
+                        double *L, double *R, double *roe) {
+  eigensystem(gamma, QL, QR, nhat, L, R, roe);
+}
+
+double oracle_d1(const double *f, int32_t n, int32_t i, int32_t per, double delta) {
+  return d1_line(f, 1, n, i, per != 0, delta);
+}
+double oracle_d2(const double *f, int32_t n, int32_t i, int32_t per, double delta) {
+  return d2_line(f, 1, n, i, per != 0, delta);
+}
+
+int32_t oracle_halo(const oracle_params *p, int32_t *h) {
+  const Grid g = make_grid(p);
+  for (int d = 0; d < 3; ++d) h[d] = g.h[d];
+  return 0;
+}
+int64_t oracle_field_size(const oracle_params *p) { return make_grid(p).total; }
+
+void oracle_interface_flux(const oracle_params *p, const double *Q, int32_t dir,
+                           int32_t i, int32_t j, int32_t k, double *fhat, double *margin) {
+  const Grid g = make_grid(p);
+  interface_flux(p, g, Q, dir, g.idx(i, j, k), fhat, margin);
+}
+
+int32_t oracle_bc(const oracle_params *p, double *Q) {
+  if (validate(p)) return 1;
+  const Grid g = make_grid(p);
+  for (int d = 0; d < 3; ++d) bc_direction(p, g, Q, d);
+  return 0;
+}
+
+int32_t oracle_rhs(const oracle_params *p, const double *Q, double *R, int32_t parts, double *margin) {
+  if (validate(p)) return 1;
+  const Grid g = make_grid(p);
+  rhs_full(p, g, Q, R, parts, margin);
+  return 0;
+}
+
+int32_t oracle_rhs_points(const oracle_params *p, const double *Q, int32_t parts,
+                          int64_t npts, const int32_t *ijk, double *out) {
+  if (validate(p)) return 1;
+  const Grid g = make_grid(p);
+  PrimSource ps{p, &g, Q, nullptr};
+#pragma omp parallel for num_threads(p->nthreads) schedule(dynamic, 16)
+  for (int64_t t = 0; t < npts; ++t) {
+    const int i = ijk[3 * t], j = ijk[3 * t + 1], k = ijk[3 * t + 2];
+    const long at = g.idx(i, j, k);
+    double r[5] = {0, 0, 0, 0, 0};
+    if (parts & ORACLE_PART_INVISCID) {
+      for (int d = 0; d < 3; ++d) {
+        if (!g.active(d)) continue;
+        double fp[5], fm[5];
+        interface_flux(p, g, Q, d, at, fp, nullptr);
+        interface_flux(p, g, Q, d, at - g.stride(d), fm, nullptr);
+        const double div = flux_divisor(p, d, at);
+        for (int c = 0; c < 5; ++c) r[c] -= (fp[c] - fm[c]) / div;
+      }
+    }
+    if ((parts & ORACLE_PART_VISCOUS) && p->visc != ORACLE_VISC_NONE) {
+      double rv[5] = {0, 0, 0, 0, 0};
+      viscous_at(ps, NodeIdx{{i, j, k}}, at, rv);
+      for (int c = 1; c < 5; ++c) r[c] += rv[c];
+    }
+    for (int c = 0; c < 5; ++c) out[5 * t + c] = r[c];
+  }
+  return 0;
+}
+
+int32_t oracle_metrics(const oracle_params *p, const double *coords,
+                       double *const *D, double *detJ, double *const *E) {
+  if (validate(p)) return 1;
+  const Grid g = make_grid(p);
+  metrics_from_coords(p, g, coords, D, detJ, E);
+  return 0;
+}
+
+/* PAPER.md:232-242 eq. (36)-(38); coefficients of the 3-stage scheme of ref. [23]
+ * (Williamson's 2N-storage RK3, Q15). */
+void oracle_rk3_update(int32_t s, double dt, int64_t count, double *U, double *dU, const double *R) {
+  const double A[3] = {0.0, -5.0 / 9.0, -153.0 / 128.0};
+  const double B[3] = {1.0 / 3.0, 15.0 / 16.0, 8.0 / 15.0};
+  for (int64_t o = 0; o < count; ++o) {
+    /* A_0 = 0: dU^(0) is never read, so it need not be initialised */
+    const double du = (s == 0 ? 0.0 : A[s] * dU[o]) + dt * R[o];               /* eq. (36) */
+    dU[o] = du;
+    U[o] = U[o] + B[s] * du;                                                    /* eq. (37) */
+  }
+}
+
+int32_t oracle_rk3_step(const oracle_params *p, double *Q, double *dU, double *R, double dt) {
+  if (validate(p)) return 1;
+  const Grid g = make_grid(p);
+  for (int s = 0; s < 3; ++s) {
+    for (int d = 0; d < 3; ++d) bc_direction(p, g, Q, d);
+    rhs_full(p, g, Q, R, ORACLE_PART_INVISCID | ORACLE_PART_VISCOUS, nullptr);
+    /* stage update on interior nodes, one x-line at a time */
+#pragma omp parallel for num_threads(p->nthreads) schedule(static)
+    for (int k = 0; k < g.n[2]; ++k)
+      for (int j = 0; j < g.n[1]; ++j)
+        for (int c = 0; c < 5; ++c) {
+          const long o = c * g.total + g.idx(0, j, k);
+          oracle_rk3_update(s, dt, g.n[0], Q + o, dU + o, R + o);
+        }
+  }
+  for (int d = 0; d < 3; ++d) bc_direction(p, g, Q, d);
+  return 0;
+}
+
+}  // extern "C"

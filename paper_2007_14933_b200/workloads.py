@@ -1,0 +1,185 @@
+"""Seeded, synthetic input generators for the five BASELINE.json configurations (+ pin cases).
+
+This module holds NO arithmetic of the method (no reconstruction, no flux, no difference
+stencil, no boundary formula): it only evaluates analytic initial fields and grid coordinates
+and packs them.  It is the one module both the CPU oracle's tests and the CUDA path's
+tests/bench import, so that both sides receive identical bytes.
+
+Exchange format ("dense padded"): a scalar field is a float64 array [NZ, NY, NX] with
+N_d = n_d + 2 h_d, h_d = 3 if n_d > 1 else 0; a state is [5, NZ, NY, NX] holding
+(rho, rho u, rho v, rho w, rho E).  Halo entries of an initial state are an
+edge copy (they are overwritten by the first boundary fill).
+
+Recipes: DESIGN.md "Input recipe"; PAPER.md:469-479 (Sod), 497-511 (Euler wave on the
+sinusoidal mesh), 623 (Taylor-Green vortex), 576-601 (SBLI set-up the slab case is modelled on).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import Optional
+
+import numpy as np
+
+WENOZ5, TENO5 = 0, 1
+VISC_NONE, VISC_CONST, VISC_SUTHERLAND = 0, 1, 2
+BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL = 0, 1, 2, 3
+
+
+@dataclass
+class Case:
+    name: str
+    n: tuple                                   # (nx, ny, nz)
+    Q0: np.ndarray                             # [5, NZ, NY, NX] dense padded
+    dt: float
+    nsteps: int
+    delta: tuple = (1.0, 1.0, 1.0)             # uniform spacing (uniform mode)
+    coords: Optional[np.ndarray] = None        # [3, NZ, NY, NX] node coordinates => curvilinear mode
+    gamma: float = 1.4
+    Re: float = 1.0
+    Pr: float = 1.0
+    Minf: float = 1.0
+    scheme: int = WENOZ5
+    teno_ct: float = 1e-6
+    eps: float = 1e-16
+    visc: int = VISC_NONE
+    suth_ratio: float = 110.4 / 288.0
+    bc: tuple = ((0, 0), (0, 0), (0, 0))
+    wall_T: tuple = ((0.0, 0.0), (0.0, 0.0), (0.0, 0.0))
+    dirichlet: Optional[np.ndarray] = None     # [5, NZ, NY, NX] frozen boundary state
+    extra: dict = field(default_factory=dict)  # analytic solutions etc. for the pins
+
+    @property
+    def halo(self):
+        return tuple(3 if v > 1 else 0 for v in self.n)
+
+    @property
+    def periodic(self):
+        return tuple(self.bc[d][0] == BC_PERIODIC for d in range(3))
+
+    @property
+    def npoints(self):
+        return int(self.n[0]) * int(self.n[1]) * int(self.n[2])
+
+    def physics(self):
+        """Keyword arguments shared by both back-ends' constructors (metrics excluded)."""
+        return dict(n=self.n, delta=self.delta, gamma=self.gamma, Re=self.Re, Pr=self.Pr, Minf=self.Minf,
+                    scheme=self.scheme, teno_ct=self.teno_ct, eps=self.eps, visc=self.visc,
+                    suth_ratio=self.suth_ratio, bc=self.bc, wall_T=self.wall_T, dirichlet=self.dirichlet)
+
+
+# ------------------------------------------------------------------------------ helpers ----
+def halo_of(n):
+    return tuple(3 if v > 1 else 0 for v in n)
+
+
+def padded_index_grids(n):
+    """Integer node indices (i, j, k) on the dense padded grid, as broadcastable arrays."""
+    h = halo_of(n)
+    i = np.arange(-h[0], n[0] + h[0])[None, None, :]
+    j = np.arange(-h[1], n[1] + h[1])[None, :, None]
+    k = np.arange(-h[2], n[2] + h[2])[:, None, None]
+    return i, j, k
+
+
+def conservative(rho, u, v, w, p, gamma):
+    """Pack primitive fields into the 5-variable conservative state (eq. 7)."""
+    shape = np.broadcast_shapes(*(np.shape(a) for a in (rho, u, v, w, p)))
+    rho, u, v, w, p = (np.broadcast_to(np.asarray(a, dtype=np.float64), shape) for a in (rho, u, v, w, p))
+    Q = np.empty((5,) + shape)
+    Q[0] = rho
+    Q[1] = rho * u
+    Q[2] = rho * v
+    Q[3] = rho * w
+    Q[4] = p / (gamma - 1.0) + 0.5 * rho * (u * u + v * v + w * w)
+    return Q
+
+
+def edge_pad_interior(A, n):
+    """Overwrite halo entries of dense padded array(s) [..., NZ, NY, NX] by an edge copy."""
+    h = halo_of(n)
+    core = A[..., h[2]:h[2] + n[2], h[1]:h[1] + n[1], h[0]:h[0] + n[0]]
+    pw = [(0, 0)] * (A.ndim - 3) + [(h[2],) * 2, (h[1],) * 2, (h[0],) * 2]
+    return np.ascontiguousarray(np.pad(core, pw, mode="edge"))
+
+
+def splitmix64_unit(seed, index):
+    """Counter-based uniform numbers in [-1, 1): splitmix64(seed + index) -> top 53 bits."""
+    z = (np.asarray(index, dtype=np.uint64) + np.uint64(seed)) + np.uint64(0x9E3779B97F4A7C15)
+    z = (z ^ (z >> np.uint64(30))) * np.uint64(0xBF58476D1CE4E5B9)
+    z = (z ^ (z >> np.uint64(27))) * np.uint64(0x94D049BB133111EB)
+    z = z ^ (z >> np.uint64(31))
+    return (z >> np.uint64(11)).astype(np.float64) / float(1 << 52) - 1.0
+
+
+# --------------------------------------------------------------------------------- C1 ------
+def sod(nx=400, scheme=WENOZ5, dt=2e-4, nsteps=1000):
+    """1-D Sod shock tube (BASELINE.json config 1).  x_i = i/(nx-1)."""
+    n = (nx, 1, 1)
+    i, _, _ = padded_index_grids(n)
+    x = i / (nx - 1.0)
+    left = x < 0.5
+    rho = np.where(left, 1.0, 0.125)
+    p = np.where(left, 1.0, 0.1)
+    Q0 = conservative(rho, 0.0, 0.0, 0.0, p, 1.4)
+    Q0 = edge_pad_interior(Q0, n)
+    return Case(name=f"sod{nx}", n=n, Q0=Q0, dt=dt, nsteps=nsteps, delta=(1.0 / (nx - 1.0), 1.0, 1.0),
+                gamma=1.4, Minf=1.0, scheme=scheme, visc=VISC_NONE,
+                bc=((BC_EXTRAP0, BC_EXTRAP0), (0, 0), (0, 0)),
+                extra={"x": np.arange(nx) / (nx - 1.0), "t_end": dt * nsteps})
+
+
+# ----------------------------------------------------------------------------- C2/C3/C5 ----
+_TGV_DT = {64: (3.385e-3, 100), 256: (8.5e-4, 200), 512: (4.2e-4, 50)}
+
+
+def tgv(n=64, scheme=TENO5, visc=VISC_CONST, dt=None, nsteps=None, M=0.1, Re=1600.0, Pr=0.71):
+    """3-D viscous Taylor-Green vortex on [0, 2 pi)^3 (BASELINE.json configs 2, 3, 5)."""
+    nn = (n, n, n)
+    i, j, k = padded_index_grids(nn)
+    h = 2.0 * np.pi / n
+    x, y, z = i * h, j * h, k * h
+    gamma = 1.4
+    u = np.sin(x) * np.cos(y) * np.cos(z)
+    v = -np.cos(x) * np.sin(y) * np.cos(z)
+    p = 1.0 / (gamma * M * M) + (np.cos(2 * x) + np.cos(2 * y)) * (np.cos(2 * z) + 2.0) / 16.0
+    rho = gamma * M * M * p
+    Q0 = np.ascontiguousarray(conservative(rho, u, v, 0.0, p, gamma))
+    if dt is None or nsteps is None:
+        d0, s0 = _TGV_DT.get(n, (3.385e-3 * 64.0 / n, 10))
+        dt = d0 if dt is None else dt
+        nsteps = s0 if nsteps is None else nsteps
+    per = (BC_PERIODIC, BC_PERIODIC)
+    return Case(name=f"tgv{n}", n=nn, Q0=Q0, dt=dt, nsteps=nsteps, delta=(h, h, h), gamma=gamma, Re=Re, Pr=Pr,
+                Minf=M, scheme=scheme, visc=visc, bc=(per, per, per))
+
+
+# ------------------------------------------------------------- Euler wave, sinusoidal mesh --
+def euler_wave(N=32, scheme=WENOZ5, A=0.04, dt=5e-4, t_end=2.5, curvilinear=True):
+    """2-D travelling density wave on the sinusoidal mesh (eq. 47-49).
+
+    rho = 1 + 0.2 sin(pi (x + y - t (u + v))), u = 1, v = -0.5, p = 1; periodic, L_x = L_y = 2.
+    """
+    n = (N, N, 1)
+    i, j, k = padded_index_grids(n)
+    L = 2.0
+    d = L / N
+    x = i * d + A * np.sin(6.0 * np.pi * j * d / L) + 0.0 * k
+    y = j * d + A * np.sin(6.0 * np.pi * i * d / L) + 0.0 * k
+    if not curvilinear:
+        x = i * d + 0.0 * j + 0.0 * k
+        y = j * d + 0.0 * i + 0.0 * k
+    u0, v0, p0, gamma = 1.0, -0.5, 1.0, 1.4
+
+    def rho_exact(xx, yy, t):
+        return 1.0 + 0.2 * np.sin(np.pi * (xx + yy - t * (u0 + v0)))
+
+    Q0 = np.ascontiguousarray(conservative(rho_exact(x, y, 0.0), u0, v0, 0.0, p0, gamma))
+    coords = np.ascontiguousarray(np.stack([x, y, np.zeros_like(x)])) if curvilinear else None
+    per = (BC_PERIODIC, BC_PERIODIC)
+    nsteps = int(round(t_end / dt))
+    h = halo_of(n)
+    xi = x[:, h[1]:h[1] + N, h[0]:h[0] + N]
+    yi = y[:, h[1]:h[1] + N, h[0]:h[0] + N]
+    return Case(name=f"wave{N}", n=n, Q0=Q0, dt=dt, nsteps=nsteps, delta=(d, d, 1.0), coords=coords, gamma=gamma,
+                Minf=1.0, scheme=scheme, visc=VISC_NONE, bc=(per, per, (0, 0)),
+                extra={"rho_exact": rho_exact(xi, yi, dt * nsteps), "t_end": dt * nsteps})
