@@ -1,0 +1,294 @@
+// osbli_api.cu -- host side of the C ABI declared in include/osbli.h: layout, parameter
+// validation, launch sequencing on the caller's stream.  No device allocation, no synchronisation
+// (except osbli_advance_host), no CPU fallback.
+#include "../../include/osbli.h"
+#include "osbli_kernels.h"
+
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace osbli;
+
+struct ProfiledLaunch { int cls; cudaEvent_t t0, t1; };
+
+struct osbli_ctx {
+  DevParams P;
+  double *R;          // residual state in the workspace (used by osbli_rk3_step)
+  double *prim;       // staged u, v, w, T (, mu) fields in the workspace
+  int64_t launches;
+  bool profiling;
+  std::vector<ProfiledLaunch> *prof;   // events around every launch while profiling
+};
+
+namespace {
+
+int make_layout(const osbli_params *p, Layout *L) {
+  const int n[3] = {p->nx, p->ny, p->nz};
+  for (int d = 0; d < 3; ++d) {
+    if (n[d] < 1) return OSBLI_EINVAL;
+    if (n[d] > 1 && n[d] < 5) return OSBLI_EINVAL;
+    L->n[d] = n[d];
+    L->h[d] = n[d] > 1 ? kHalo : 0;
+  }
+  L->xoff = kXOffset;
+  const long long rowlen = kXOffset + (long long)n[0] + kXTail;
+  L->sy = (rowlen + 15) / 16 * 16;
+  L->sz = L->sy * (n[1] + 2 * L->h[1]);
+  L->sv = L->sz * (n[2] + 2 * L->h[2]);
+  return OSBLI_OK;
+}
+
+int nprim(const osbli_params *p) {
+  return p->visc == OSBLI_VISC_NONE ? 0 : (p->visc == OSBLI_VISC_SUTHERLAND ? 5 : 4);
+}
+
+int validate(const osbli_params *p) {
+  if (!p) return OSBLI_EINVAL;
+  Layout L;
+  if (int rc = make_layout(p, &L)) return rc;
+  if (p->nx == 1) return OSBLI_EUNSUPPORTED;                       // x is the contiguous direction; it must be active
+  if (p->scheme != OSBLI_SCHEME_WENOZ5 && p->scheme != OSBLI_SCHEME_TENO5) return OSBLI_EINVAL;
+  if (p->visc < OSBLI_VISC_NONE || p->visc > OSBLI_VISC_SUTHERLAND) return OSBLI_EINVAL;
+  if (!(p->gamma > 1.0)) return OSBLI_EINVAL;
+  if (!(p->eps >= 1e-18) || !(p->teno_ct > 0.0)) return OSBLI_EINVAL;
+  if (p->visc != OSBLI_VISC_NONE && (!(p->Re > 0.0) || !(p->Pr > 0.0) || !(p->Minf > 0.0))) return OSBLI_EINVAL;
+  bool need_dirichlet = false;
+  for (int d = 0; d < 3; ++d) {
+    const int n = d == 0 ? p->nx : (d == 1 ? p->ny : p->nz);
+    for (int s = 0; s < 2; ++s) {
+      const int b = p->bc[d][s];
+      if (b < OSBLI_BC_PERIODIC || b > OSBLI_BC_WALL_ISOTHERMAL) return OSBLI_EINVAL;
+      if (n > 1 && b == OSBLI_BC_DIRICHLET) need_dirichlet = true;
+      if (n > 1 && b == OSBLI_BC_WALL_ISOTHERMAL && !(p->wall_T[d][s] > 0.0)) return OSBLI_EINVAL;
+      if (n > 1 && b == OSBLI_BC_WALL_ISOTHERMAL && !(p->Minf > 0.0)) return OSBLI_EINVAL;
+    }
+    if ((p->bc[d][0] == OSBLI_BC_PERIODIC) != (p->bc[d][1] == OSBLI_BC_PERIODIC)) return OSBLI_EINVAL;
+  }
+  if (need_dirichlet && !p->dirichlet) return OSBLI_EINVAL;
+  if (!p->metrics) {
+    const double dl[3] = {p->dx, p->dy, p->dz};
+    for (int d = 0; d < 3; ++d)
+      if (L.n[d] > 1 && !(dl[d] > 0.0)) return OSBLI_EINVAL;
+  } else {
+    const osbli_metrics *m = p->metrics;
+    if (!m->detJ) return OSBLI_EINVAL;
+    for (int k = 0; k < 3; ++k) {
+      for (int j = 0; j < 3; ++j)
+        if (!m->D[k][j]) return OSBLI_EINVAL;
+      if (p->visc != OSBLI_VISC_NONE)
+        for (int e = 0; e < 6; ++e)
+          if (!m->E[k][e]) return OSBLI_EINVAL;
+    }
+  }
+  return OSBLI_OK;
+}
+
+inline cudaStream_t as_stream(void *s) { return reinterpret_cast<cudaStream_t>(s); }
+
+// Every kernel launch goes through here: counted, and (only while osbli_profile_begin is in
+// effect) bracketed by two events on the same stream so that bench.py can attribute device time
+// to kernel classes without a profiler attached.
+#define OSBLI_LAUNCH(h, cls, st, call)                                   \
+  do {                                                                   \
+    ProfiledLaunch pl_ = {cls, nullptr, nullptr};                        \
+    if ((h)->profiling) {                                                \
+      if (cudaEventCreate(&pl_.t0) != cudaSuccess || cudaEventCreate(&pl_.t1) != cudaSuccess) return OSBLI_ECUDA; \
+      cudaEventRecord(pl_.t0, st);                                       \
+    }                                                                    \
+    if ((call) != cudaSuccess) return OSBLI_ECUDA;                       \
+    if ((h)->profiling) { cudaEventRecord(pl_.t1, st); (h)->prof->push_back(pl_); } \
+    ++(h)->launches;                                                     \
+  } while (0)
+
+int do_bc(osbli_ctx *h, double *Q, cudaStream_t st) {
+  for (int d = 0; d < 3; ++d)
+    if (h->P.L.n[d] > 1) OSBLI_LAUNCH(h, OSBLI_K_BC, st, launch_bc(h->P, d, Q, st));
+  return OSBLI_OK;
+}
+
+int do_rhs(osbli_ctx *h, const double *Q, double *R, cudaStream_t st) {
+  const DevParams &P = h->P;
+  if (P.visc != OSBLI_VISC_NONE) OSBLI_LAUNCH(h, OSBLI_K_PRIM, st, launch_primitives(P, Q, h->prim, st));
+  int accumulate = 0;
+  for (int d = 0; d < 3; ++d) {
+    if (P.L.n[d] <= 1) continue;
+    OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep(P, d, Q, R, accumulate, st));
+    accumulate = 1;
+  }
+  if (P.visc != OSBLI_VISC_NONE) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, accumulate, st));
+  return OSBLI_OK;
+}
+
+int do_step(osbli_ctx *h, double *Q, double *Qtmp, double dt, cudaStream_t st) {
+  for (int s = 0; s < 3; ++s) {
+    if (int rc = do_bc(h, Q, st)) return rc;
+    if (int rc = do_rhs(h, Q, h->R, st)) return rc;
+    OSBLI_LAUNCH(h, OSBLI_K_RK, st, launch_rk_update(h->P, s, dt, Q, Qtmp, h->R, st));
+  }
+  return do_bc(h, Q, st);
+}
+
+}  // namespace
+
+extern "C" {
+
+int osbli_get_layout(const osbli_params *p, osbli_layout *out) {
+  if (!p || !out) return OSBLI_EINVAL;
+  Layout L;
+  if (int rc = make_layout(p, &L)) return rc;
+  for (int d = 0; d < 3; ++d) out->halo[d] = L.h[d];
+  out->x_offset = L.xoff;
+  out->stride_y = L.sy;
+  out->stride_z = L.sz;
+  out->stride_var = L.sv;
+  out->total_doubles = 5 * L.sv;
+  return OSBLI_OK;
+}
+
+int osbli_workspace_bytes(const osbli_params *p, size_t *out) {
+  if (!p || !out) return OSBLI_EINVAL;
+  Layout L;
+  if (int rc = make_layout(p, &L)) return rc;
+  if (p->visc < OSBLI_VISC_NONE || p->visc > OSBLI_VISC_SUTHERLAND) return OSBLI_EINVAL;
+  *out = (size_t)(5 + nprim(p)) * (size_t)L.sv * sizeof(double);
+  return OSBLI_OK;
+}
+
+int osbli_init(const osbli_params *p, void *d_workspace, size_t workspace_bytes, osbli_handle *out) {
+  if (!out) return OSBLI_EINVAL;
+  *out = nullptr;
+  if (int rc = validate(p)) return rc;
+  size_t need = 0;
+  osbli_workspace_bytes(p, &need);
+  if (!d_workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(d_workspace) & 255u)) return OSBLI_EWORKSPACE;
+
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return OSBLI_ECUDA;
+  if (prop.major != 10) return OSBLI_ECUDA;                      // sm_100a code only; no other path exists
+
+  osbli_ctx *h = new (std::nothrow) osbli_ctx;
+  if (!h) return OSBLI_EINVAL;
+  std::memset(h, 0, sizeof(*h));
+  DevParams &P = h->P;
+  make_layout(p, &P.L);
+  P.curvilinear = p->metrics ? 1 : 0;
+  const double dl[3] = {p->dx, p->dy, p->dz};
+  for (int d = 0; d < 3; ++d) {
+    const double delta = (P.L.n[d] > 1 && !P.curvilinear) ? dl[d] : 1.0;
+    P.inv_delta[d] = 1.0 / delta;
+    P.inv12d[d] = 1.0 / (12.0 * delta);
+    P.inv12d2[d] = 1.0 / (12.0 * delta * delta);
+    P.periodic[d] = p->bc[d][0] == OSBLI_BC_PERIODIC;
+    for (int s = 0; s < 2; ++s) { P.bc[d][s] = p->bc[d][s]; P.wall_T[d][s] = p->wall_T[d][s]; }
+  }
+  P.gamma = p->gamma; P.gm1 = p->gamma - 1.0;
+  P.Re = p->Re; P.inv_Re = p->visc != OSBLI_VISC_NONE ? 1.0 / p->Re : 0.0;
+  P.Pr = p->Pr; P.Minf = p->Minf; P.gM2 = p->gamma * p->Minf * p->Minf;
+  P.cq = p->visc != OSBLI_VISC_NONE ? 1.0 / ((p->gamma - 1.0) * p->Minf * p->Minf * p->Pr * p->Re) : 0.0;
+  P.scheme = p->scheme; P.visc = p->visc;
+  P.ct = p->teno_ct; P.eps = p->eps; P.suth = p->suth_ratio;
+  P.dirichlet = p->dirichlet;
+  if (p->metrics) {
+    for (int k = 0; k < 3; ++k) {
+      for (int j = 0; j < 3; ++j) P.D[k][j] = p->metrics->D[k][j];
+      for (int e = 0; e < 6; ++e) P.E[k][e] = p->metrics->E[k][e];
+    }
+    P.detJ = p->metrics->detJ;
+  }
+  h->prof = new (std::nothrow) std::vector<ProfiledLaunch>();
+  if (!h->prof) { delete h; return OSBLI_EINVAL; }
+  h->R = static_cast<double *>(d_workspace);
+  h->prim = h->R + 5 * P.L.sv;
+  *out = h;
+  return OSBLI_OK;
+}
+
+int osbli_bc(osbli_handle h, double *d_Q, void *cuda_stream) {
+  if (!h || !d_Q) return OSBLI_EINVAL;
+  return do_bc(h, d_Q, as_stream(cuda_stream));
+}
+
+int osbli_rhs(osbli_handle h, const double *d_Q, double *d_R, void *cuda_stream) {
+  if (!h || !d_Q || !d_R || d_Q == d_R) return OSBLI_EINVAL;
+  return do_rhs(h, d_Q, d_R, as_stream(cuda_stream));
+}
+
+int osbli_rk3_step(osbli_handle h, double *d_Q, double *d_Qtmp, double dt, void *cuda_stream) {
+  if (!h || !d_Q || !d_Qtmp || d_Q == d_Qtmp) return OSBLI_EINVAL;
+  return do_step(h, d_Q, d_Qtmp, dt, as_stream(cuda_stream));
+}
+
+int osbli_advance_host(osbli_handle h, double *h_Q, double *d_Q, double *d_Qtmp, double dt, int32_t nsteps,
+                       void *cuda_stream) {
+  if (!h || !h_Q || !d_Q || !d_Qtmp || d_Q == d_Qtmp || nsteps < 0) return OSBLI_EINVAL;
+  cudaStream_t st = as_stream(cuda_stream);
+  const size_t bytes = (size_t)5 * (size_t)h->P.L.sv * sizeof(double);
+  if (cudaMemcpyAsync(d_Q, h_Q, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return OSBLI_ECUDA;
+  for (int s = 0; s < nsteps; ++s)
+    if (int rc = do_step(h, d_Q, d_Qtmp, dt, st)) return rc;
+  if (cudaMemcpyAsync(h_Q, d_Q, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return OSBLI_ECUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return OSBLI_ECUDA;
+  return OSBLI_OK;
+}
+
+int osbli_launch_count(osbli_handle h, int64_t *out) {
+  if (!h || !out) return OSBLI_EINVAL;
+  *out = h->launches;
+  return OSBLI_OK;
+}
+
+int osbli_profile_begin(osbli_handle h) {
+  if (!h || h->profiling) return OSBLI_EINVAL;
+  h->profiling = true;
+  return OSBLI_OK;
+}
+
+int osbli_profile_end(osbli_handle h, void *cuda_stream, double *ms_per_class, int64_t *launches_per_class) {
+  if (!h || !h->profiling || !ms_per_class || !launches_per_class) return OSBLI_EINVAL;
+  h->profiling = false;
+  int rc = OSBLI_OK;
+  if (cudaStreamSynchronize(as_stream(cuda_stream)) != cudaSuccess) rc = OSBLI_ECUDA;
+  for (int c = 0; c < OSBLI_K_COUNT; ++c) { ms_per_class[c] = 0.0; launches_per_class[c] = 0; }
+  for (ProfiledLaunch &pl : *h->prof) {
+    float ms = 0.f;
+    if (rc == OSBLI_OK && cudaEventElapsedTime(&ms, pl.t0, pl.t1) != cudaSuccess) rc = OSBLI_ECUDA;
+    ms_per_class[pl.cls] += ms;
+    ++launches_per_class[pl.cls];
+    cudaEventDestroy(pl.t0);
+    cudaEventDestroy(pl.t1);
+  }
+  h->prof->clear();
+  return rc;
+}
+
+int osbli_measure_fp64_peak(void *d_scratch, void *cuda_stream, double *tflops) {
+  if (!d_scratch || !tflops) return OSBLI_EINVAL;
+  return measure_fp64_peak(static_cast<double *>(d_scratch), as_stream(cuda_stream), tflops) == cudaSuccess
+             ? OSBLI_OK : OSBLI_ECUDA;
+}
+
+int osbli_destroy(osbli_handle h) {
+  if (!h) return OSBLI_EINVAL;
+  if (h->prof) {
+    for (ProfiledLaunch &pl : *h->prof) { cudaEventDestroy(pl.t0); cudaEventDestroy(pl.t1); }
+    delete h->prof;
+  }
+  delete h;
+  return OSBLI_OK;
+}
+
+const char *osbli_strerror(int status) {
+  switch (status) {
+    case OSBLI_OK: return "ok";
+    case OSBLI_EINVAL: return "invalid argument";
+    case OSBLI_EUNSUPPORTED: return "unsupported configuration";
+    case OSBLI_ECUDA: return "CUDA error (no sm_100 device, or a launch / copy failed)";
+    case OSBLI_EWORKSPACE: return "workspace missing, too small or not 256-byte aligned";
+    default: return "unknown status";
+  }
+}
+
+}  // extern "C"

@@ -1,0 +1,23 @@
+// osbli_kernels.h -- host-side launchers of the CUDA kernels (internal to libosbli).
+#pragma once
+#include "osbli_common.cuh"
+
+namespace osbli {
+
+// R (-)= flux difference of the characteristic reconstruction along `dir` (osbli_sweep.cu)
+cudaError_t launch_sweep(const DevParams &P, int dir, const double *Q, double *R, int accumulate, cudaStream_t st);
+
+// staged primitive fields u, v, w, T (, mu) on the halo-extended grid, then R += viscous terms (osbli_visc.cu)
+cudaError_t launch_primitives(const DevParams &P, const double *Q, double *prim, cudaStream_t st);
+cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *prim, double *R, int accumulate, cudaStream_t st);
+
+// halo fill along one direction (osbli_bc_rk.cu); returns the number of launches through *nl
+cudaError_t launch_bc(const DevParams &P, int dir, double *Q, cudaStream_t st);
+
+// RK3 stage update, eq. (36)-(37): Qtmp = A Qtmp + dt R; Q += B Qtmp on interior nodes
+cudaError_t launch_rk_update(const DevParams &P, int stage, double dt, double *Q, double *Qtmp, const double *R, cudaStream_t st);
+
+// DFMA micro-benchmark (osbli_peak.cu): measured fp64 TFLOP/s of this device; d_scratch >= 8 bytes
+cudaError_t measure_fp64_peak(double *d_scratch, cudaStream_t st, double *tflops);
+
+}  // namespace osbli

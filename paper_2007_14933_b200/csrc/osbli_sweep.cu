@@ -1,0 +1,278 @@
+// osbli_sweep.cu -- per-direction characteristic reconstruction sweeps (PAPER.md:100-111 steps 1-4,
+// eq. (10)): R (-)= (f^_{i+1/2} - f^_{i-1/2}) / Delta_d   (or / detJ_i on curvilinear grids).
+//
+// Design ("marching"): every thread owns one grid line segment along the sweep direction and
+// walks along it with a 6-point register window of staged point states.  Each point's
+// thermodynamics (step 1) is computed once per sweep, each interface flux (step 2) once, and the
+// previous interface flux stays in registers for the difference (step 3) -- no redundant work
+// apart from a 5-point warm-up and one extra flux per segment.
+//   * y, z sweeps: thread <-> x index, so every global access of a warp is a contiguous row
+//     segment (coalesced, 128-byte aligned rows).
+//   * x sweep: lane <-> line (32 consecutive (j,k) lines per warp).  Rows are moved in 8-point
+//     tiles through warp-private shared memory (a 32 x 8 transpose, padded to stride 9), so global
+//     traffic stays in whole 64-byte segments and nothing needs a block-wide barrier.
+#include "osbli_flux.cuh"
+#include "osbli_kernels.h"
+
+namespace osbli {
+
+// ---------------------------------------------------------------------------------------------
+// y / z sweeps
+// ---------------------------------------------------------------------------------------------
+template <int DIR, int SCHEME, bool CURV>
+__global__ void __launch_bounds__(128)
+sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
+                int chunk, int accumulate) {
+  static_assert(DIR == 1 || DIR == 2, "x has its own kernel");
+  const Layout &Ly = P.L;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= Ly.n[0]) return;
+  const int t = blockIdx.y;                      // transverse index: k for the y sweep, j for the z sweep
+  const int n = Ly.n[DIR];
+  const int s0 = blockIdx.z * chunk;
+  const int s1 = min(s0 + chunk, n);
+  const long long st = (DIR == 1) ? Ly.sy : Ly.sz;
+  const long long line0 = (DIR == 1) ? Ly.at(i, 0, t) : Ly.at(i, t, 0);   // node 0 of this line
+  const long long sv = Ly.sv;
+  const double eps12 = 48.0 * P.eps;
+  const double inv_d = P.inv_delta[DIR];
+
+  Pt<CURV> w[6];
+  double rsq[3] = {1.0, 1.0, 1.0};               // 1/sqrt(rho) of window slots 3, 4, 5
+  RoeSide rl = {0, 0, 0, 0, 0};
+  double prev[5] = {0, 0, 0, 0, 0};
+
+  auto load = [&](int node, double (&q)[5], double (&K)[3]) {
+    const long long o = line0 + (long long)node * st;
+#pragma unroll
+    for (int c = 0; c < 5; ++c) q[c] = __ldg(Q + c * sv + o);
+    if constexpr (CURV) {
+      const double J = __ldg(P.detJ + o);
+      K[0] = J * __ldg(P.D[DIR][0] + o);
+      K[1] = J * __ldg(P.D[DIR][1] + o);
+      K[2] = J * __ldg(P.D[DIR][2] + o);
+    } else {
+      K[0] = K[1] = K[2] = 0.0;
+    }
+  };
+
+  // warm-up: nodes s0-3 .. s0+1 into slots 1..5 (after the first shift they sit in 0..4)
+#pragma unroll
+  for (int m = 1; m < 6; ++m) {
+    double q[5], K[3];
+    load(s0 - 4 + m, q, K);
+    double rs;
+    make_point<DIR, CURV>(P, q[0], q[1], q[2], q[3], q[4], K[0], K[1], K[2], w[m], rs);
+    if (m >= 3) rsq[m - 3] = rs;
+    if (m == 3) rl = roe_side<CURV>(w[3], rs);   // node s0-1 = left node of the first interface
+  }
+  double qn[5], Kn[3];
+  load(s0 + 2, qn, Kn);                          // prefetched raw state of the next node
+
+  for (int q = s0 - 1; q < s1; ++q) {            // interface q+1/2, between nodes q and q+1
+#pragma unroll
+    for (int m = 0; m < 5; ++m) w[m] = w[m + 1];
+    rsq[0] = rsq[1]; rsq[1] = rsq[2];
+    make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], w[5], rsq[2]);
+    if (q + 1 < s1) load(q + 4, qn, Kn);         // node (q+1)+3, used by the next interface
+    const RoeSide rr = roe_side<CURV>(w[3], rsq[0]);
+    double f[5];
+    if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, rl, rr, eps12, f);
+    else interface_flux<DIR, SCHEME>(P, w, rl, rr, eps12, f);
+    rl = rr;
+    if (q >= s0) {
+      const long long o = line0 + (long long)q * st;
+      double sc = inv_d;
+      if constexpr (CURV) sc = 1.0 / __ldg(P.detJ + o);
+#pragma unroll
+      for (int c = 0; c < 5; ++c) {
+        const double dr = (prev[c] - f[c]) * sc;
+        double *dst = R + c * sv + o;
+        *dst = accumulate ? (*dst + dr) : dr;
+      }
+    }
+#pragma unroll
+    for (int c = 0; c < 5; ++c) prev[c] = f[c];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// x sweep
+// ---------------------------------------------------------------------------------------------
+constexpr int kXT = 8;                 // points per transposed tile
+constexpr int kXP = kXT + 1;           // padded row stride in shared memory (bank-conflict free)
+constexpr int kXWarps = 4;             // warps per block
+
+template <bool CURV> struct XSmem {
+  double in[CURV ? 9 : 5][32][kXP];    // staged rows: 5 conservative variables (+ detJ, K_x, K_y, K_z)
+  double out[5][32][kXP];              // staged flux differences
+};
+
+template <int SCHEME, bool CURV>
+__global__ void __launch_bounds__(kXWarps * 32)
+sweep_x_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
+               int chunk, int accumulate) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const Layout &Ly = P.L;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  XSmem<CURV> &S = reinterpret_cast<XSmem<CURV> *>(smem_raw)[warp];
+  const int nlines = Ly.n[1] * Ly.n[2];
+  const int line0 = (blockIdx.x * kXWarps + warp) * 32;
+  if (line0 >= nlines) return;                                   // whole warp leaves together
+  const int line = min(line0 + lane, nlines - 1);                // clamp: idle lanes mirror the last line
+  const bool live = (line0 + lane) < nlines;
+  const long long row = Ly.at(0, line % Ly.n[1], line / Ly.n[1]);   // node 0 of my line
+  const long long sv = Ly.sv;
+  const int nx = Ly.n[0];
+  const int s0 = blockIdx.y * chunk;                             // chunk is a multiple of kXT
+  const int s1 = min(s0 + chunk, nx);
+  const double eps12 = 48.0 * P.eps;
+  const double inv_d = P.inv_delta[0];
+  constexpr int NIN = CURV ? 9 : 5;
+
+  // cooperative tile load: 32 rows x 8 points, each instruction moves 4 rows of 64 bytes
+  const int lr = lane >> 3, lc = lane & 7;
+  auto load_tile = [&](int a) {                                  // points [a, a+8), a multiple of 8
+#pragma unroll
+    for (int it = 0; it < 8; ++it) {
+      const int rr_ = it * 4 + lr;
+      const long long ro = __shfl_sync(0xffffffffu, row, rr_) + a + lc;
+#pragma unroll
+      for (int c = 0; c < 5; ++c) S.in[c][rr_][lc] = __ldg(Q + c * sv + ro);
+      if constexpr (CURV) {
+        S.in[5][rr_][lc] = __ldg(P.detJ + ro);
+        S.in[6][rr_][lc] = __ldg(P.D[0][0] + ro);
+        S.in[7][rr_][lc] = __ldg(P.D[0][1] + ro);
+        S.in[8][rr_][lc] = __ldg(P.D[0][2] + ro);
+      }
+    }
+  };
+  auto store_tile = [&](int a) {                                 // flux differences of points [a, a+8) ∩ [s0, s1)
+#pragma unroll
+    for (int it = 0; it < 8; ++it) {
+      const int rr_ = it * 4 + lr;
+      const long long ro = __shfl_sync(0xffffffffu, row, rr_) + a + lc;
+      const bool ok = (line0 + rr_ < nlines) && (a + lc < s1);
+      if (ok) {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {
+          double *dst = R + c * sv + ro;
+          const double v = S.out[c][rr_][lc];
+          *dst = accumulate ? (*dst + v) : v;
+        }
+      }
+    }
+  };
+
+  Pt<CURV> w[6];
+  double rsq[3] = {1.0, 1.0, 1.0};
+  double Jw[4] = {1.0, 1.0, 1.0, 1.0};           // detJ of window slots 2..5 (curvilinear divisor)
+  RoeSide rl = {0, 0, 0, 0, 0};
+  double prev[5] = {0, 0, 0, 0, 0};
+#pragma unroll
+  for (int m = 0; m < 6; ++m) { w[m].r = 1.0; w[m].m[0] = w[m].m[1] = w[m].m[2] = 0.0; w[m].E = 1.0; w[m].p = 1.0; w[m].th = 0.0; w[m].c = 1.0; }
+
+  int a_in = ((s0 - 3) >= 0) ? ((s0 - 3) / kXT) * kXT : -kXT;    // tile holding node s0-3 (s0-3 >= -3)
+  load_tile(a_in);
+  __syncwarp();
+
+  for (int node = s0 - 3; node < s1 + 3; ++node) {               // node entering window slot 5
+    if (node >= a_in + kXT) {
+      __syncwarp();
+      a_in += kXT;
+      load_tile(a_in);
+      __syncwarp();
+    }
+    const int col = node - a_in;
+#pragma unroll
+    for (int m = 0; m < 5; ++m) w[m] = w[m + 1];
+    rsq[0] = rsq[1]; rsq[1] = rsq[2];
+    Jw[0] = Jw[1]; Jw[1] = Jw[2]; Jw[2] = Jw[3];
+    {
+      const double r = S.in[0][lane][col], mx = S.in[1][lane][col], my = S.in[2][lane][col];
+      const double mz = S.in[3][lane][col], E = S.in[4][lane][col];
+      double kx = 0.0, ky = 0.0, kz = 0.0;
+      if constexpr (CURV) {
+        const double J = S.in[5][lane][col];
+        kx = J * S.in[6][lane][col]; ky = J * S.in[7][lane][col]; kz = J * S.in[8][lane][col];
+        Jw[3] = J;
+      }
+      make_point<0, CURV>(P, r, mx, my, mz, E, kx, ky, kz, w[5], rsq[2]);
+    }
+    const int q = node - 3;                                      // interface q+1/2 is now computable
+    if (q == s0 - 2) rl = roe_side<CURV>(w[3], rsq[0]);         // slot 3 holds node s0-1
+    if (q < s0 - 1) continue;
+    const RoeSide rr = roe_side<CURV>(w[3], rsq[0]);
+    double f[5];
+    if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, rl, rr, eps12, f);
+    else interface_flux<0, SCHEME>(P, w, rl, rr, eps12, f);
+    rl = rr;
+    if (q >= s0) {
+      double sc = inv_d;
+      if constexpr (CURV) sc = 1.0 / Jw[0];                      // slot 2 = node q
+      const int oc = q & (kXT - 1);
+#pragma unroll
+      for (int c = 0; c < 5; ++c) S.out[c][lane][oc] = (prev[c] - f[c]) * sc;
+      if (oc == kXT - 1 || q == s1 - 1) {
+        __syncwarp();
+        store_tile(q - oc);
+        __syncwarp();
+      }
+    }
+#pragma unroll
+    for (int c = 0; c < 5; ++c) prev[c] = f[c];
+  }
+  (void)live;
+}
+
+// ---------------------------------------------------------------------------------------------
+// host-side launchers
+// ---------------------------------------------------------------------------------------------
+template <int SCHEME, bool CURV>
+static cudaError_t launch_x(const DevParams &P, const double *Q, double *R, int accumulate, cudaStream_t st) {
+  const int nlines = P.L.n[1] * P.L.n[2];
+  const int nx = P.L.n[0];
+  int chunk = 64;
+  if (nx <= 64) chunk = ((nx + kXT - 1) / kXT) * kXT;
+  dim3 grid((nlines + kXWarps * 32 - 1) / (kXWarps * 32), (nx + chunk - 1) / chunk, 1);
+  const size_t smem = sizeof(XSmem<CURV>) * kXWarps;
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaError_t e = cudaFuncSetAttribute(sweep_x_kernel<SCHEME, CURV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_done = true;
+  }
+  sweep_x_kernel<SCHEME, CURV><<<grid, kXWarps * 32, smem, st>>>(P, Q, R, chunk, accumulate);
+  return cudaGetLastError();
+}
+
+template <int DIR, int SCHEME, bool CURV>
+static cudaError_t launch_yz(const DevParams &P, const double *Q, double *R, int accumulate, cudaStream_t st) {
+  const int nx = P.L.n[0];
+  const int n = P.L.n[DIR];
+  const int nt = (DIR == 1) ? P.L.n[2] : P.L.n[1];
+  const int bx = nx >= 128 ? 128 : (nx > 64 ? 128 : (nx > 32 ? 64 : 32));
+  int chunk = n > 64 ? 32 : n;
+  dim3 grid((nx + bx - 1) / bx, nt, (n + chunk - 1) / chunk);
+  sweep_yz_kernel<DIR, SCHEME, CURV><<<grid, bx, 0, st>>>(P, Q, R, chunk, accumulate);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_sweep(const DevParams &P, int dir, const double *Q, double *R, int accumulate, cudaStream_t st) {
+  const bool curv = P.curvilinear != 0;
+  const int sch = P.scheme;
+#define OSBLI_DISPATCH(SCH, CRV)                                              \
+  if (sch == SCH && curv == CRV) {                                            \
+    if (dir == 0) return launch_x<SCH, CRV>(P, Q, R, accumulate, st);         \
+    if (dir == 1) return launch_yz<1, SCH, CRV>(P, Q, R, accumulate, st);     \
+    return launch_yz<2, SCH, CRV>(P, Q, R, accumulate, st);                   \
+  }
+  OSBLI_DISPATCH(0, false)
+  OSBLI_DISPATCH(1, false)
+  OSBLI_DISPATCH(0, true)
+  OSBLI_DISPATCH(1, true)
+#undef OSBLI_DISPATCH
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace osbli

@@ -183,3 +183,67 @@ def euler_wave(N=32, scheme=WENOZ5, A=0.04, dt=5e-4, t_end=2.5, curvilinear=True
     return Case(name=f"wave{N}", n=n, Q0=Q0, dt=dt, nsteps=nsteps, delta=(d, d, 1.0), coords=coords, gamma=gamma,
                 Minf=1.0, scheme=scheme, visc=VISC_NONE, bc=(per, per, (0, 0)),
                 extra={"rho_exact": rho_exact(xi, yi, dt * nsteps), "t_end": dt * nsteps})
+
+
+# --------------------------------------------------- small curvilinear box (parity cases) ----
+def wavy_box(n=(24, 20, 8), seed=1, bc=None, scheme=WENOZ5, visc=VISC_SUTHERLAND, M=2.0, Re=950.0, Pr=0.72,
+             amp=0.05, grid_amp=0.03, wall_T=1.2, dt=1e-3, nsteps=2):
+    """Smooth seeded flow on a smooth fully 3-D curvilinear mapping; any mix of boundary types.
+
+    Not one of the paper's cases: a small stand-in with the structure of the SBLI slab (curvilinear
+    metrics incl. cross terms, Sutherland viscosity, wall / Dirichlet / extrapolation / periodic
+    boundaries) that the oracle finishes in seconds.  Coordinates are analytic in the node index, so
+    halo coordinates are the periodic continuation where a direction is periodic.
+    """
+    n = tuple(int(v) for v in n)
+    if bc is None:
+        bc = ((BC_DIRICHLET, BC_EXTRAP0), (BC_WALL_ISOTHERMAL, BC_DIRICHLET), (BC_PERIODIC, BC_PERIODIC))
+    per = tuple(bc[d][0] == BC_PERIODIC for d in range(3))
+    rng = np.random.default_rng(seed)
+    i, j, k = padded_index_grids(n)
+    # computational coordinates in [0,1): periodic directions use n points per period, others n-1 intervals
+    den = [float(n[d] if per[d] else max(n[d] - 1, 1)) for d in range(3)]
+    xi, et, ze = i / den[0] + 0.0 * j + 0.0 * k, j / den[1] + 0.0 * i + 0.0 * k, k / den[2] + 0.0 * i + 0.0 * j
+    Lx, Ly, Lz = 2.0, 1.5, 1.0
+    tw = 2.0 * np.pi
+    active = [v > 1 for v in n]
+    bump = np.sin(tw * xi) * (np.sin(tw * et) if active[1] else 1.0) * (np.cos(tw * ze) if active[2] else 1.0)
+    x = Lx * (xi + grid_amp * bump)
+    y = Ly * (et + grid_amp * np.sin(tw * xi + 0.3) * np.sin(tw * et)) if active[1] else 0.0 * xi
+    z = Lz * (ze + grid_amp * np.sin(tw * ze) * np.cos(tw * xi)) if active[2] else 0.0 * xi
+    coords = np.ascontiguousarray(np.stack([x, y, z]))
+    ph = rng.uniform(0, tw, size=12)
+    gamma = 1.4
+    p0 = 1.0 / (gamma * M * M)
+
+    def wave(a, b, c, q):
+        return np.sin(tw * (a * xi + b * et + c * ze) + q)
+
+    rho = 1.0 + amp * wave(1, 1, 1, ph[0]) + 0.5 * amp * wave(2, 0, 1, ph[1])
+    u = 1.0 + amp * wave(1, 2, 0, ph[2])
+    v = amp * wave(2, 1, 1, ph[3]) if active[1] else 0.0 * xi
+    w = amp * wave(1, 1, 2, ph[4]) if active[2] else 0.0 * xi
+    p = p0 * (1.0 + amp * wave(1, 1, 1, ph[5]) + 0.5 * amp * wave(0, 2, 1, ph[6]))
+    Q0 = np.ascontiguousarray(conservative(rho, u, v, w, p, gamma))
+    dirichlet = Q0.copy()
+    wt = tuple(tuple(wall_T if bc[d][s] == BC_WALL_ISOTHERMAL else 0.0 for s in range(2)) for d in range(3))
+    return Case(name="wavy_box", n=n, Q0=Q0, dt=dt, nsteps=nsteps, delta=(1.0, 1.0, 1.0), coords=coords, gamma=gamma,
+                Re=Re, Pr=Pr, Minf=M, scheme=scheme, visc=visc, bc=bc, wall_T=wt, dirichlet=dirichlet)
+
+
+def perturb(case, seed=0, amp=0.02):
+    """Seeded perturbation of a case's initial state (rho, p stay > 0); returns a new dense Q0.
+
+    Moves parity inputs away from the symmetric analytic fields, where many terms vanish.
+    Momentum along an inactive direction stays exactly zero (Q27)."""
+    rng = np.random.default_rng(seed)
+    Q = case.Q0.copy()
+    h = case.halo
+    core = (slice(h[2], h[2] + case.n[2]), slice(h[1], h[1] + case.n[1]), slice(h[0], h[0] + case.n[0]))
+    for c in range(5):
+        if c in (1, 2, 3) and case.n[c - 1] == 1:
+            continue
+        ref = np.abs(Q[c][core]).max()
+        scale = amp * (0.1 * ref if c in (0, 4) else max(ref, 0.1))
+        Q[c][core] += scale * rng.uniform(-1.0, 1.0, size=Q[c][core].shape)
+    return edge_pad_interior(Q, case.n)

@@ -1,0 +1,149 @@
+"""Helpers shared by the GPU parity tests: build the oracle and the CUDA solver from one Case,
+norms, and the tolerance model of DESIGN.md "Tolerances".
+
+Tolerance on a single residual evaluation (per variable c, absolute):
+
+    tol_c = max( 1e-11 * den_c ,  K_ULP * 2^-53 * max_nodes( Phi_c * sum_d |grad xi_d| ) )
+
+* first term: north_star's "max relative difference <= 1e-11", relative in the sense of DESIGN.md
+  Q28 (den_c = ||R_c||_inf of the oracle, or the largest such norm if variable c is ~0);
+* second term: the fp64 rounding floor of the residual itself.  R is a difference of interface
+  fluxes divided by the spacing, and each interface flux is a sum of characteristic contributions
+  of magnitude up to Phi_c = (|u|+a)|Q_c| (+ p for momentum, + (|u|+a) p for energy).  At low Mach
+  number Phi_c/Delta is ~1e5-1e6 times ||R_c||, so 1e-11 relative is below one rounding error of
+  the terms being subtracted: the oracle compiled with FMA contraction (same source, same
+  operation order) already differs from itself by 3.7e-11 on the 64^3 TGV, i.e. ~3 of these units
+  (tests/test_tolerance_floor.py pins that on the CPU).  K_ULP = 32 such units are allowed.
+On the well-conditioned cases (Sod, Mach-2 boxes) the first term is the larger one and the stated
+1e-11 applies unchanged.
+"""
+from __future__ import annotations
+
+import json
+import os
+from pathlib import Path
+
+import numpy as np
+
+from oracle import oracle as O
+
+K_ULP = 32.0
+U = 2.0 ** -53
+REL = 1e-11
+
+_REPORT = Path(__file__).resolve().parent.parent / "gpurun_out" / "parity_report.jsonl"
+
+
+def report(**kw):
+    """Append one JSON line to gpurun_out/parity_report.jsonl (best effort; never fails a test)."""
+    try:
+        _REPORT.parent.mkdir(exist_ok=True)
+        with open(_REPORT, "a") as f:
+            f.write(json.dumps(kw, default=float) + "\n")
+    except Exception:
+        pass
+
+
+def metrics_for(case):
+    if case.coords is None:
+        return None
+    return O.metrics_from_coords(case.coords, case.n, case.periodic, delta=case.delta)
+
+
+def make_oracle(case, metrics=None, **over):
+    kw = case.physics()
+    kw.update(over)
+    return O.Oracle(metrics=metrics, **kw)
+
+
+def make_solver(case, metrics=None, **over):
+    from paper_2007_14933_b200 import osbli
+    kw = case.physics()
+    kw.update(over)
+    return osbli.Solver(metrics=metrics, **kw)
+
+
+def interior(case, A):
+    h = case.halo
+    n = case.n
+    return A[..., h[2]:h[2] + n[2], h[1]:h[1] + n[1], h[0]:h[0] + n[0]]
+
+
+def q28(a, b):
+    """DESIGN.md Q28: per variable max|a-b| / den_c, den_c = ||b_c||_inf (or the largest one if ~0)."""
+    S = max(float(np.abs(b[c]).max()) for c in range(5))
+    out = []
+    for c in range(5):
+        den = float(np.abs(b[c]).max())
+        if den < 1e-12 * S:
+            den = S
+        out.append(float(np.abs(a[c] - b[c]).max()) / den if den > 0 else 0.0)
+    return out
+
+
+def l1_rel(a, b):
+    S = max(float(np.abs(b[c]).max()) for c in range(5))
+    out = []
+    for c in range(5):
+        den = float(np.abs(b[c]).max())
+        if den < 1e-12 * S:
+            den = S
+        out.append(float(np.abs(a[c] - b[c]).mean()) / den if den > 0 else 0.0)
+    return out
+
+
+def flux_scale(case, Qi, metrics=None, points=None):
+    """max over (the given) interior nodes of Phi_c * sum_d |grad xi_d|; Qi = interior state [5,nz,ny,nx]."""
+    g = case.gamma
+    rho = Qi[0]
+    u, v, w = Qi[1] / rho, Qi[2] / rho, Qi[3] / rho
+    p = (g - 1.0) * (Qi[4] - 0.5 * rho * (u * u + v * v + w * w))
+    a = np.sqrt(g * p / rho)
+    speed = np.sqrt(u * u + v * v + w * w) + a
+    geo = np.zeros_like(rho)
+    for d in range(3):
+        if case.n[d] <= 1:
+            continue
+        if metrics is None:
+            geo = geo + 1.0 / case.delta[d]
+        else:
+            D = [interior(case, metrics["D"][d][j]) for j in range(3)]
+            geo = geo + np.sqrt(D[0] ** 2 + D[1] ** 2 + D[2] ** 2)
+    phi = [speed * np.abs(Qi[0]),
+           speed * np.abs(Qi[1]) + p, speed * np.abs(Qi[2]) + p, speed * np.abs(Qi[3]) + p,
+           speed * (np.abs(Qi[4]) + p)]
+    return np.array([float((f * geo).max()) for f in phi])
+
+
+def residual_tolerance(case, Qi, Ro_i, metrics=None):
+    """Absolute per-variable tolerance for one residual evaluation (see module docstring)."""
+    S = max(float(np.abs(Ro_i[c]).max()) for c in range(5))
+    den = np.array([float(np.abs(Ro_i[c]).max()) for c in range(5)])
+    den = np.where(den < 1e-12 * S, S, den)
+    floor = K_ULP * U * flux_scale(case, Qi, metrics)
+    return np.maximum(REL * den, floor), REL * den, floor
+
+
+def check_residual(name, case, Qi, Rg_i, Ro_i, metrics=None, margin_i=None, margin_min=1e-9):
+    """Assert GPU residual Rg matches oracle residual Ro on interior nodes.
+
+    Nodes whose TENO cut-off decision is within `margin_min` of flipping in the oracle
+    (Q14) are excluded from the maximum and counted."""
+    tol, tol_rel, tol_floor = residual_tolerance(case, Qi, Ro_i, metrics)
+    mask = np.ones(Ro_i.shape[1:], dtype=bool)
+    nflip = 0
+    if margin_i is not None:
+        mask = margin_i >= margin_min
+        nflip = int((~mask).sum())
+    err = np.array([float(np.abs(Rg_i[c] - Ro_i[c])[mask].max()) for c in range(5)])
+    rel = q28(np.where(mask, Rg_i, Ro_i), Ro_i)
+    report(test=name, kind="residual", err_abs=err.tolist(), tol_abs=tol.tolist(), q28=rel,
+           err_in_floor_units=(err / (tol_floor / K_ULP)).tolist(), excluded_nodes=nflip,
+           npoints=int(mask.size))
+    assert np.isfinite(Rg_i).all(), f"{name}: non-finite GPU residual"
+    assert nflip <= max(8, mask.size // 100000), f"{name}: too many near-cut-off nodes excluded ({nflip})"
+    for c in range(5):
+        assert err[c] <= tol[c], (f"{name}: variable {c}: |dR| = {err[c]:.3e} > tol {tol[c]:.3e} "
+                                  f"(1e-11 rel = {tol_rel[c]:.3e}, rounding floor x{K_ULP:g} = {tol_floor[c]:.3e}; "
+                                  f"q28 = {rel[c]:.3e})")
+    return err, tol

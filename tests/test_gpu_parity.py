@@ -1,0 +1,239 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin ctypes binding) against the CPU
+oracle, element by element on the same seeded inputs.  Tolerances: tests/parity.py (residual),
+north_star's 1e-9 (state after the configured steps, Q28 norm), L1 <= 1e-9 (shocked cases).
+"""
+import numpy as np
+import pytest
+
+import parity
+from oracle import oracle as O
+from paper_2007_14933_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def gpu_residual(sol, Qdense):
+    Q = sol.to_padded(Qdense)
+    sol.bc(Q)
+    R = sol.empty_state(0.0)
+    sol.rhs(Q, R)
+    _torch().cuda.synchronize()
+    return sol.from_padded(Q), sol.from_padded(R)
+
+
+def run_residual_case(name, case, Q0=None, **over):
+    metrics = parity.metrics_for(case)
+    orc = parity.make_oracle(case, metrics, **over)
+    sol = parity.make_solver(case, metrics, **over)
+    Q0 = case.Q0 if Q0 is None else Q0
+    Qo = orc.bc(Q0.copy())
+    scheme = over.get("scheme", case.scheme)
+    Ro, mg = orc.rhs(Qo, margin=True)
+    Qg, Rg = gpu_residual(sol, Q0)
+    # halo fill: copy-type boundaries are bit-exact; the wall formulas agree to rounding
+    has_wall = any(b == W.BC_WALL_ISOTHERMAL for d in range(3) for b in case.bc[d] if case.n[d] > 1)
+    if has_wall:
+        np.testing.assert_allclose(Qg, Qo, rtol=1e-13, atol=1e-14)
+    else:
+        assert np.array_equal(Qg, Qo), f"{name}: halo fill differs"
+    mi = parity.interior(case, mg) if scheme == W.TENO5 else None
+    parity.check_residual(name, case, parity.interior(case, Qo), parity.interior(case, Rg),
+                          parity.interior(case, Ro), metrics, margin_i=mi)
+    sol.close()
+
+
+# ------------------------------------------------------------------------------ residual ----
+def test_residual_sod_initial_and_developed():
+    case = W.sod()
+    run_residual_case("sod_t0", case)
+    orc = parity.make_oracle(case)
+    Q = orc.run(case.Q0.copy(), case.dt, 150)
+    run_residual_case("sod_t0.03", case, Q0=Q)
+    run_residual_case("sod_t0.03_teno", case, Q0=Q, scheme=W.TENO5)
+
+
+@pytest.mark.parametrize("scheme", [W.TENO5, W.WENOZ5])
+@pytest.mark.parametrize("visc", [W.VISC_NONE, W.VISC_CONST])
+def test_residual_tgv32(scheme, visc):
+    case = W.tgv(32, scheme=scheme, visc=visc)
+    run_residual_case(f"tgv32_s{scheme}_v{visc}", case)
+    run_residual_case(f"tgv32_s{scheme}_v{visc}_perturbed", case, Q0=W.perturb(case, seed=5, amp=0.05))
+
+
+def test_residual_tgv64_config2():
+    run_residual_case("tgv64", W.tgv(64))
+
+
+def test_residual_ragged_sizes_span_tiles():
+    """Sizes that are not multiples of any tile: several x chunks (64), y/z chunks (32) and ragged tails."""
+    case = W.tgv(16)
+    big = W.Case(**{**case.__dict__})
+    n = (70, 37, 35)
+    i, j, k = W.padded_index_grids(n)
+    x, y, z = 2 * np.pi * i / n[0], 2 * np.pi * j / n[1], 2 * np.pi * k / n[2]
+    g, M = 1.4, 0.4
+    u = np.sin(x) * np.cos(y) * np.cos(z)
+    v = -np.cos(x) * np.sin(y) * np.cos(z)
+    w = 0.3 * np.sin(x + y) * np.sin(z)
+    p = 1.0 / (g * M * M) + (np.cos(2 * x) + np.cos(2 * y)) * (np.cos(2 * z) + 2.0) / 16.0
+    rho = 1.0 + 0.2 * np.sin(x + 2 * y - z)
+    big.n = n
+    big.Q0 = np.ascontiguousarray(W.conservative(rho, u, v, w, p, g))
+    big.delta = tuple(2 * np.pi / v_ for v_ in n)
+    big.Minf = M
+    big.Re = 100.0
+    big.name = "ragged"
+    run_residual_case("ragged_teno", big)
+    run_residual_case("ragged_wenoz_perturbed", big, Q0=W.perturb(big, seed=9, amp=0.05), scheme=W.WENOZ5)
+
+
+def test_residual_2d_and_nonperiodic_closures():
+    """nz = 1 (inactive direction), extrapolation boundaries -> one-sided closures eq. (30)-(35)."""
+    n = (40, 33, 1)
+    i, j, k = W.padded_index_grids(n)
+    x, y = i / (n[0] - 1.0) + 0 * j + 0 * k, j / (n[1] - 1.0) + 0 * i + 0 * k
+    g, M = 1.4, 0.8
+    rho = 1.0 + 0.1 * np.sin(3 * x) * np.cos(2 * y)
+    u = 0.5 + 0.2 * np.sin(2 * x + y)
+    v = 0.1 * np.cos(3 * x - 2 * y)
+    p = 1.0 / (g * M * M) * (1.0 + 0.1 * np.cos(2 * x + 3 * y))
+    Q0 = np.ascontiguousarray(W.conservative(rho, u, v, 0.0, p, g))
+    ex = (W.BC_EXTRAP0, W.BC_EXTRAP0)
+    case = W.Case(name="box2d", n=n, Q0=Q0, dt=1e-3, nsteps=1, delta=(1.0 / (n[0] - 1), 1.0 / (n[1] - 1), 1.0),
+                  gamma=g, Re=200.0, Pr=0.72, Minf=M, scheme=W.WENOZ5, visc=W.VISC_SUTHERLAND, bc=(ex, ex, (0, 0)))
+    run_residual_case("box2d_extrap_sutherland", case)
+    run_residual_case("box2d_extrap_const_teno", case, visc=W.VISC_CONST, scheme=W.TENO5)
+
+
+def test_residual_curvilinear_euler_wave():
+    run_residual_case("wave32", W.euler_wave(32))
+    run_residual_case("wave48_teno", W.euler_wave(48, scheme=W.TENO5))
+
+
+@pytest.mark.parametrize("scheme", [W.WENOZ5, W.TENO5])
+def test_residual_curvilinear_3d_walls_sutherland(scheme):
+    case = W.wavy_box(n=(70, 21, 9), scheme=scheme)
+    run_residual_case(f"wavy_box_s{scheme}", case)
+
+
+def test_residual_curvilinear_3d_periodic_const_visc():
+    per = (W.BC_PERIODIC, W.BC_PERIODIC)
+    case = W.wavy_box(n=(24, 20, 12), bc=(per, per, per), visc=W.VISC_CONST, M=0.5)
+    run_residual_case("wavy_box_periodic", case)
+
+
+# ----------------------------------------------------------------------------- RK3 steps ----
+def run_steps_case(name, case, nsteps, tol, norm, **over):
+    metrics = parity.metrics_for(case)
+    orc = parity.make_oracle(case, metrics, **over)
+    sol = parity.make_solver(case, metrics, **over)
+    Qo = orc.run(case.Q0.copy(), case.dt, nsteps)
+    Q = sol.to_padded(case.Q0)
+    Qtmp = sol.empty_state()
+    for _ in range(nsteps):
+        sol.rk3_step(Q, Qtmp, case.dt)
+    _torch().cuda.synchronize()
+    Qg = sol.from_padded(Q)
+    a, b = parity.interior(case, Qg), parity.interior(case, Qo)
+    err = norm(a, b)
+    parity.report(test=name, kind="state", nsteps=nsteps, err=err, tol=tol)
+    assert np.isfinite(Qg).all()
+    assert max(err) <= tol, (name, err)
+    # halos after the final bc agree as well
+    assert max(parity.q28(Qg, Qo)) <= max(tol, 1e-12)
+    sol.close()
+    return Qg, Qo
+
+
+def test_steps_sod_config1_full():
+    """BASELINE.json config 1: 1000 steps, L1 <= 1e-9 (shocked case)."""
+    case = W.sod()
+    run_steps_case("sod_1000", case, case.nsteps, 1e-9, parity.l1_rel)
+
+
+def test_steps_tgv32_short():
+    case = W.tgv(32)
+    run_steps_case("tgv32_10", case, 10, 1e-9, parity.q28)
+
+
+def test_steps_tgv64_config2_full():
+    """BASELINE.json config 2: 100 steps at 64^3, max relative difference <= 1e-9."""
+    case = W.tgv(64)
+    run_steps_case("tgv64_100", case, case.nsteps, 1e-9, parity.q28)
+
+
+def test_steps_curvilinear_walls():
+    case = W.wavy_box(n=(40, 21, 9))
+    run_steps_case("wavy_box_5", case, 5, 1e-9, parity.l1_rel)
+
+
+def test_advance_host_matches_device_steps():
+    case = W.tgv(32)
+    sol = parity.make_solver(case)
+    Q = sol.to_padded(case.Q0)
+    Qtmp = sol.empty_state()
+    for _ in range(3):
+        sol.rk3_step(Q, Qtmp, case.dt)
+    hQ = sol.to_padded(case.Q0, pinned_host=True)
+    Q2, Qtmp2 = sol.empty_state(), sol.empty_state()
+    sol.advance_host(hQ, Q2, Qtmp2, case.dt, 3)
+    assert np.array_equal(sol.from_padded(hQ), sol.from_padded(Q))
+    assert sol.launch_count() > 0
+    sol.close()
+
+
+# ------------------------------------------------- full size, bench launch configuration ----
+def sampled_full_size(name, n, nsamples, presteps):
+    """At BASELINE.json's full sizes the oracle is evaluated one node at a time on sampled nodes
+    (oracle_rhs_points) of the state the GPU produced after `presteps` steps."""
+    torch = _torch()
+    case = W.tgv(n)
+    sol = parity.make_solver(case)
+    Q = sol.to_padded(case.Q0)
+    Qtmp = sol.empty_state()
+    for _ in range(presteps):
+        sol.rk3_step(Q, Qtmp, case.dt)
+    R = Qtmp                               # reuse as the residual buffer
+    sol.rhs(Q, R)
+    torch.cuda.synchronize()
+    Qd = sol.from_padded(Q)
+    Rd = sol.from_padded(R)
+    del Q, Qtmp, R
+    assert np.isfinite(parity.interior(case, Rd)).all()
+    rng = np.random.default_rng(2007)
+    ijk = np.stack([rng.integers(0, n, nsamples) for _ in range(3)], axis=1).astype(np.int32)
+    # always include corners / edges / tile seams
+    seams = np.array([[0, 0, 0], [n - 1, n - 1, n - 1], [0, n - 1, 31], [63, 32, 0], [64, 31, n - 1], [n - 1, 0, 32]],
+                     dtype=np.int32)
+    ijk = np.concatenate([seams, ijk])
+    orc = parity.make_oracle(case)
+    Ro = orc.rhs_points(Qd, ijk)           # [npts, 5]
+    h = case.halo
+    Rg = np.stack([Rd[:, ijk[t, 2] + h[2], ijk[t, 1] + h[1], ijk[t, 0] + h[0]] for t in range(len(ijk))])
+    Qi = parity.interior(case, Qd)
+    # tolerance from the oracle's whole-field scale is not available at this size: use the sampled maxima
+    fake_R = Ro.T.reshape(5, 1, 1, -1)
+    tol, tol_rel, floor = parity.residual_tolerance(case, Qi, fake_R)
+    err = np.abs(Rg - Ro).max(axis=0)
+    parity.report(test=name, kind="sampled_residual", err_abs=err.tolist(), tol_abs=tol.tolist(),
+                  err_in_floor_units=(err / (floor / parity.K_ULP)).tolist(), nsamples=len(ijk))
+    assert (err <= tol).all(), (name, err, tol)
+    sol.close()
+
+
+def test_full_size_tgv256_config3_sampled():
+    sampled_full_size("tgv256_sampled", 256, 3000, presteps=2)
+
+
+def test_full_size_tgv512_config5_sampled():
+    torch = _torch()
+    free, total = torch.cuda.mem_get_info()
+    import psutil
+    if free < 60e9 or psutil.virtual_memory().available < 40e9:
+        pytest.skip("not enough device / host memory for the 512^3 case")
+    sampled_full_size("tgv512_sampled", 512, 1500, presteps=1)
