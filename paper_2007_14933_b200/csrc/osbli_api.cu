@@ -110,14 +110,16 @@ int do_bc(osbli_ctx *h, double *Q, cudaStream_t st) {
 
 int do_rhs(osbli_ctx *h, const double *Q, double *R, cudaStream_t st) {
   const DevParams &P = h->P;
-  if (P.visc != OSBLI_VISC_NONE) OSBLI_LAUNCH(h, OSBLI_K_PRIM, st, launch_primitives(P, Q, h->prim, st));
+  const bool fast_visc = viscous_fast_path(P);
+  if (P.visc != OSBLI_VISC_NONE && !fast_visc) OSBLI_LAUNCH(h, OSBLI_K_PRIM, st, launch_primitives(P, Q, h->prim, st));
   int accumulate = 0;
   for (int d = 0; d < 3; ++d) {
     if (P.L.n[d] <= 1) continue;
     OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep(P, d, Q, R, accumulate, st));
     accumulate = 1;
   }
-  if (P.visc != OSBLI_VISC_NONE) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, accumulate, st));
+  if (fast_visc) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous_fast(P, Q, R, st));
+  else if (P.visc != OSBLI_VISC_NONE) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, accumulate, st));
   return OSBLI_OK;
 }
 

@@ -11,6 +11,10 @@ cudaError_t launch_sweep(const DevParams &P, int dir, const double *Q, double *R
 cudaError_t launch_primitives(const DevParams &P, const double *Q, double *prim, cudaStream_t st);
 cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *prim, double *R, int accumulate, cudaStream_t st);
 
+// fused fast path (uniform grid, mu = 1, three periodic directions): reads Q directly, R += viscous terms
+bool viscous_fast_path(const DevParams &P);
+cudaError_t launch_viscous_fast(const DevParams &P, const double *Q, double *R, cudaStream_t st);
+
 // halo fill along one direction (osbli_bc_rk.cu); returns the number of launches through *nl
 cudaError_t launch_bc(const DevParams &P, int dir, double *Q, cudaStream_t st);
 

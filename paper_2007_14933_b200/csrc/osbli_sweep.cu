@@ -19,10 +19,10 @@ namespace osbli {
 // ---------------------------------------------------------------------------------------------
 // y / z sweeps
 // ---------------------------------------------------------------------------------------------
-template <int DIR, int SCHEME, bool CURV>
+template <int DIR, int SCHEME, bool CURV, bool ACCUM>
 __global__ void __launch_bounds__(128)
 sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
-                int chunk, int accumulate) {
+                int chunk) {
   static_assert(DIR == 1 || DIR == 2, "x has its own kernel");
   const Layout &Ly = P.L;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -75,6 +75,15 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
     rsq[0] = rsq[1]; rsq[1] = rsq[2];
     make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], w[5], rsq[2]);
     if (q + 1 < s1) load(q + 4, qn, Kn);         // node (q+1)+3, used by the next interface
+    // R of node q is read now and consumed after the flux: its latency hides behind ~1000 DFMAs
+    double rold[5] = {0, 0, 0, 0, 0};
+    if constexpr (ACCUM) {
+      if (q >= s0) {
+        const long long o = line0 + (long long)q * st;
+#pragma unroll
+        for (int c = 0; c < 5; ++c) rold[c] = R[c * sv + o];
+      }
+    }
     const RoeSide rr = roe_side<CURV>(w[3], rsq[0]);
     double f[5];
     if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, rl, rr, eps12, f);
@@ -85,11 +94,7 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
       double sc = inv_d;
       if constexpr (CURV) sc = 1.0 / __ldg(P.detJ + o);
 #pragma unroll
-      for (int c = 0; c < 5; ++c) {
-        const double dr = (prev[c] - f[c]) * sc;
-        double *dst = R + c * sv + o;
-        *dst = accumulate ? (*dst + dr) : dr;
-      }
+      for (int c = 0; c < 5; ++c) R[c * sv + o] = fma(prev[c] - f[c], sc, rold[c]);
     }
 #pragma unroll
     for (int c = 0; c < 5; ++c) prev[c] = f[c];
@@ -128,7 +133,6 @@ sweep_x_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q
   const int s1 = min(s0 + chunk, nx);
   const double eps12 = 48.0 * P.eps;
   const double inv_d = P.inv_delta[0];
-  constexpr int NIN = CURV ? 9 : 5;
 
   // cooperative tile load: 32 rows x 8 points, each instruction moves 4 rows of 64 bytes
   const int lr = lane >> 3, lc = lane & 7;
@@ -254,7 +258,8 @@ static cudaError_t launch_yz(const DevParams &P, const double *Q, double *R, int
   const int bx = nx >= 128 ? 128 : (nx > 64 ? 128 : (nx > 32 ? 64 : 32));
   int chunk = n > 64 ? 32 : n;
   dim3 grid((nx + bx - 1) / bx, nt, (n + chunk - 1) / chunk);
-  sweep_yz_kernel<DIR, SCHEME, CURV><<<grid, bx, 0, st>>>(P, Q, R, chunk, accumulate);
+  if (accumulate) sweep_yz_kernel<DIR, SCHEME, CURV, true><<<grid, bx, 0, st>>>(P, Q, R, chunk);
+  else sweep_yz_kernel<DIR, SCHEME, CURV, false><<<grid, bx, 0, st>>>(P, Q, R, chunk);
   return cudaGetLastError();
 }
 

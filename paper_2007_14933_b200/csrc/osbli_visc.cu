@@ -242,4 +242,196 @@ cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *pr
   return cudaGetLastError();
 }
 
+// =============================================================================================
+// Fast path: uniform grid, mu = 1, three active periodic directions (the Taylor-Green cases).
+//
+// 2.5-D marching: a block owns a 32 x 8 (x,y) tile and walks along z.  Each new z-plane of
+// u, v, w, T (tile + 2-deep x/y halo, computed from Q on the fly: no staged primitive arrays, no
+// extra HBM pass) goes into a 4-slot shared-memory ring; a thread keeps 5-deep z-windows of its own
+// column in registers: u, v, w, T for the z-derivatives, and d_x u, d_y v, d_x w, d_y w so that the
+// x-z / y-z mixed derivatives are z-differences of its own registers.  Only the x-y mixed
+// derivatives and the in-plane stencils read shared memory (84 LDS.64 per node).  One barrier per
+// plane.  R is read at the top of a step and written at its end.
+// =============================================================================================
+constexpr int kVX = 32, kVY = 8, kVH = 2;
+constexpr int kVPX = kVX + 2 * kVH, kVPY = kVY + 2 * kVH;        // 36 x 12 plane tile
+constexpr int kVRing = 4;
+
+struct VSmem { double f[kVRing][4][kVPY][kVPX]; };
+
+__global__ void __launch_bounds__(kVX * kVY, 2)
+viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
+                   int chunk) {
+  extern __shared__ __align__(16) unsigned char vs_raw[];
+  VSmem &S = *reinterpret_cast<VSmem *>(vs_raw);
+  const Layout &L = P.L;
+  const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * kVX + tx;
+  const int x0 = blockIdx.x * kVX, y0 = blockIdx.y * kVY;
+  const int z0 = blockIdx.z * chunk, z1 = min(z0 + chunk, L.n[2]);
+  const int i = x0 + tx, j = y0 + ty;
+  const bool inside = i < L.n[0] && j < L.n[1];
+  const long long sv = L.sv;
+
+  // the (up to) two tile points this thread stages per plane
+  constexpr int NPT = kVPX * kVPY;                                // 432
+  int pi[2], pj[2];
+  bool pv[2];
+#pragma unroll
+  for (int s = 0; s < 2; ++s) {
+    const int t = tid + s * (kVX * kVY);
+    pv[s] = t < NPT;
+    const int yy = pv[s] ? t / kVPX : 0, xx = pv[s] ? t % kVPX : 0;
+    pi[s] = xx; pj[s] = yy;
+    // clamp to the halo-extended domain: clamped points are never used by live threads
+    pv[s] = pv[s] && (x0 + xx - kVH) < L.n[0] + kVH && (y0 + yy - kVH) < L.n[1] + kVH;
+  }
+  auto fetch = [&](int plane, double (&q)[2][5]) {
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+      if (pv[s]) {
+        const long long at = L.at(x0 + pi[s] - kVH, y0 + pj[s] - kVH, plane);
+#pragma unroll
+        for (int c = 0; c < 5; ++c) q[s][c] = __ldg(Q + c * sv + at);
+      }
+  };
+  auto stage = [&](int plane, const double (&q)[2][5]) {
+    const int slot = (plane + 8) & (kVRing - 1);
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+      if (pv[s]) {
+        const double ir = 1.0 / q[s][0];
+        const double u = q[s][1] * ir, v = q[s][2] * ir, w = q[s][3] * ir;
+        const double p = P.gm1 * (q[s][4] - 0.5 * (q[s][1] * u + q[s][2] * v + q[s][3] * w));
+        S.f[slot][0][pj[s]][pi[s]] = u;
+        S.f[slot][1][pj[s]][pi[s]] = v;
+        S.f[slot][2][pj[s]][pi[s]] = w;
+        S.f[slot][3][pj[s]][pi[s]] = P.gM2 * p * ir;
+      }
+  };
+
+  const double cx = P.inv12d[0], cy = P.inv12d[1], cz = P.inv12d[2];
+  const double cxx = P.inv12d2[0], cyy = P.inv12d2[1], czz = P.inv12d2[2];
+  auto d1 = [](double m2, double m1, double p1, double p2, double c) { return c * ((m2 - p2) + 8.0 * (p1 - m1)); };
+  auto d2 = [](double m2, double m1, double f0, double p1, double p2, double c) {
+    return c * fma(-30.0, f0, fma(16.0, m1 + p1, -(m2 + p2)));
+  };
+
+  double uw[5], vw[5], ww[5], Tw[5], uxw[5], vyw[5], wxw[5], wyw[5];
+#pragma unroll
+  for (int m = 0; m < 5; ++m) uw[m] = vw[m] = ww[m] = Tw[m] = uxw[m] = vyw[m] = wxw[m] = wyw[m] = 0.0;
+
+  double qn[2][5];
+  fetch(z0 - 2, qn);
+  const int X = tx + kVH, Y = ty + kVH;
+
+  for (int k = z0 - 4; k < z1; ++k) {            // step k: plane k+2 enters, node k is finished
+    const int pe = k + 2;
+    const bool entering = pe >= z0 - 2;
+    if (entering) stage(pe, qn);
+    if (pe + 1 >= z0 - 2 && pe + 1 < z1 + 2) fetch(pe + 1, qn);
+    double rold[4] = {0, 0, 0, 0};
+    long long at = 0;
+    if (k >= z0 && inside) {
+      at = L.at(i, j, k);
+#pragma unroll
+      for (int c = 0; c < 4; ++c) rold[c] = R[(c + 1) * sv + at];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+      uw[m] = uw[m + 1]; vw[m] = vw[m + 1]; ww[m] = ww[m + 1]; Tw[m] = Tw[m + 1];
+      uxw[m] = uxw[m + 1]; vyw[m] = vyw[m + 1]; wxw[m] = wxw[m + 1]; wyw[m] = wyw[m + 1];
+    }
+    if (entering) {
+      const double (*F)[kVPY][kVPX] = S.f[(pe + 8) & (kVRing - 1)];
+      uw[4] = F[0][Y][X]; vw[4] = F[1][Y][X]; ww[4] = F[2][Y][X]; Tw[4] = F[3][Y][X];
+      uxw[4] = d1(F[0][Y][X - 2], F[0][Y][X - 1], F[0][Y][X + 1], F[0][Y][X + 2], cx);
+      wxw[4] = d1(F[2][Y][X - 2], F[2][Y][X - 1], F[2][Y][X + 1], F[2][Y][X + 2], cx);
+      vyw[4] = d1(F[1][Y - 2][X], F[1][Y - 1][X], F[1][Y + 1][X], F[1][Y + 2][X], cy);
+      wyw[4] = d1(F[2][Y - 2][X], F[2][Y - 1][X], F[2][Y + 1][X], F[2][Y + 2][X], cy);
+    }
+    if (k < z0 || !inside) continue;
+
+    const double (*F)[kVPY][kVPX] = S.f[(k + 8) & (kVRing - 1)];
+    // in-plane stencils of the current plane
+    const double u = uw[2], v = vw[2], w = ww[2], T = Tw[2];
+    const double uxm2 = F[0][Y][X - 2], uxm1 = F[0][Y][X - 1], uxp1 = F[0][Y][X + 1], uxp2 = F[0][Y][X + 2];
+    const double uym2 = F[0][Y - 2][X], uym1 = F[0][Y - 1][X], uyp1 = F[0][Y + 1][X], uyp2 = F[0][Y + 2][X];
+    const double vxm2 = F[1][Y][X - 2], vxm1 = F[1][Y][X - 1], vxp1 = F[1][Y][X + 1], vxp2 = F[1][Y][X + 2];
+    const double vym2 = F[1][Y - 2][X], vym1 = F[1][Y - 1][X], vyp1 = F[1][Y + 1][X], vyp2 = F[1][Y + 2][X];
+    const double u_x = uxw[2], v_y = vyw[2], w_x = wxw[2], w_y = wyw[2];
+    const double u_y = d1(uym2, uym1, uyp1, uyp2, cy);
+    const double v_x = d1(vxm2, vxm1, vxp1, vxp2, cx);
+    const double u_z = d1(uw[0], uw[1], uw[3], uw[4], cz);
+    const double v_z = d1(vw[0], vw[1], vw[3], vw[4], cz);
+    const double w_z = d1(ww[0], ww[1], ww[3], ww[4], cz);
+    const double u_xx = d2(uxm2, uxm1, u, uxp1, uxp2, cxx), u_yy = d2(uym2, uym1, u, uyp1, uyp2, cyy);
+    const double v_xx = d2(vxm2, vxm1, v, vxp1, vxp2, cxx), v_yy = d2(vym2, vym1, v, vyp1, vyp2, cyy);
+    const double u_zz = d2(uw[0], uw[1], u, uw[3], uw[4], czz);
+    const double v_zz = d2(vw[0], vw[1], v, vw[3], vw[4], czz);
+    const double w_zz = d2(ww[0], ww[1], w, ww[3], ww[4], czz);
+    const double w_xx = d2(F[2][Y][X - 2], F[2][Y][X - 1], w, F[2][Y][X + 1], F[2][Y][X + 2], cxx);
+    const double w_yy = d2(F[2][Y - 2][X], F[2][Y - 1][X], w, F[2][Y + 1][X], F[2][Y + 2][X], cyy);
+    const double T_xx = d2(F[3][Y][X - 2], F[3][Y][X - 1], T, F[3][Y][X + 1], F[3][Y][X + 2], cxx);
+    const double T_yy = d2(F[3][Y - 2][X], F[3][Y - 1][X], T, F[3][Y + 1][X], F[3][Y + 2][X], cyy);
+    const double T_zz = d2(Tw[0], Tw[1], T, Tw[3], Tw[4], czz);
+    // x-y mixed: delta_x (delta_y f), 16 points each
+    auto dxy = [&](int f) {
+      const double a2 = d1(F[f][Y - 2][X - 2], F[f][Y - 1][X - 2], F[f][Y + 1][X - 2], F[f][Y + 2][X - 2], cy);
+      const double a1 = d1(F[f][Y - 2][X - 1], F[f][Y - 1][X - 1], F[f][Y + 1][X - 1], F[f][Y + 2][X - 1], cy);
+      const double b1 = d1(F[f][Y - 2][X + 1], F[f][Y - 1][X + 1], F[f][Y + 1][X + 1], F[f][Y + 2][X + 1], cy);
+      const double b2 = d1(F[f][Y - 2][X + 2], F[f][Y - 1][X + 2], F[f][Y + 1][X + 2], F[f][Y + 2][X + 2], cy);
+      return d1(a2, a1, b1, b2, cx);
+    };
+    const double u_xy = dxy(0), v_xy = dxy(1);
+    const double u_xz = d1(uxw[0], uxw[1], uxw[3], uxw[4], cz);
+    const double w_xz = d1(wxw[0], wxw[1], wxw[3], wxw[4], cz);
+    const double v_yz = d1(vyw[0], vyw[1], vyw[3], vyw[4], cz);
+    const double w_yz = d1(wyw[0], wyw[1], wyw[3], wyw[4], cz);
+
+    const double div = u_x + v_y + w_z;
+    const double third = 1.0 / 3.0;
+    const double M0 = fma(third, u_xx + v_xy + w_xz, u_xx + u_yy + u_zz);
+    const double M1 = fma(third, u_xy + v_yy + w_yz, v_xx + v_yy + v_zz);
+    const double M2 = fma(third, u_xz + v_yz + w_zz, w_xx + w_yy + w_zz);
+    // tau_ij d_j u_i with tau = (d_j u_i + d_i u_j - 2/3 delta_ij div)/Re
+    const double t23 = (2.0 / 3.0) * div;
+    const double sxy = u_y + v_x, sxz = u_z + w_x, syz = v_z + w_y;
+    double phi = (2.0 * u_x - t23) * u_x;
+    phi = fma(2.0 * v_y - t23, v_y, phi);
+    phi = fma(2.0 * w_z - t23, w_z, phi);
+    phi = fma(sxy, sxy, phi);
+    phi = fma(sxz, sxz, phi);
+    phi = fma(syz, syz, phi);
+    const double heat = P.cq * (T_xx + T_yy + T_zz);
+    const double r1 = M0 * P.inv_Re, r2 = M1 * P.inv_Re, r3 = M2 * P.inv_Re;
+    const double r4 = fma(u, r1, fma(v, r2, w * r3)) + fma(phi, P.inv_Re, heat);
+    R[sv + at] = rold[0] + r1;
+    R[2 * sv + at] = rold[1] + r2;
+    R[3 * sv + at] = rold[2] + r3;
+    R[4 * sv + at] = rold[3] + r4;
+  }
+}
+
+bool viscous_fast_path(const DevParams &P) {
+  if (P.curvilinear || P.visc != 1) return false;
+  for (int d = 0; d < 3; ++d)
+    if (P.L.n[d] <= 1 || !P.periodic[d]) return false;
+  return true;
+}
+
+cudaError_t launch_viscous_fast(const DevParams &P, const double *Q, double *R, cudaStream_t st) {
+  const Layout &L = P.L;
+  const int chunk = L.n[2] > 64 ? 64 : L.n[2];
+  dim3 grid((L.n[0] + kVX - 1) / kVX, (L.n[1] + kVY - 1) / kVY, (L.n[2] + chunk - 1) / chunk);
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaError_t e = cudaFuncSetAttribute(viscous_tgv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(VSmem));
+    if (e != cudaSuccess) return e;
+    attr_done = true;
+  }
+  viscous_tgv_kernel<<<grid, dim3(kVX, kVY), sizeof(VSmem), st>>>(P, Q, R, chunk);
+  return cudaGetLastError();
+}
+
 }  // namespace osbli
