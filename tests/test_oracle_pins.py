@@ -56,14 +56,28 @@ def exact_riemann_sod(x, t, gamma=1.4, left=(1.0, 0.0, 1.0), right=(0.125, 0.0, 
     return rho, dict(p=p, u=us, rsl=rsl, rsr=rsr, S=S, head=head, tail=tail)
 
 
+def _golden_table(name):
+    out = {}
+    for line in (GOLDEN / name).read_text().splitlines():
+        if line.strip() and not line.startswith("#"):
+            k, v = line.split()
+            out[k] = float(v)
+    return out
+
+
 def test_p1_exact_riemann_constants():
-    """The evaluator itself against the textbook Sod constants (Toro, table 4.1 test 1 family)."""
+    """The evaluator itself against the tabulated Sod constants (tests/golden/sod_exact.txt)."""
+    g = _golden_table("sod_exact.txt")
     _, s = exact_riemann_sod(np.array([0.0]), 0.2)
-    assert abs(s["p"] - 0.303130) < 1e-6
-    assert abs(s["u"] - 0.927453) < 1e-6
-    assert abs(s["rsl"] - 0.426319) < 1e-6
-    assert abs(s["rsr"] - 0.265574) < 1e-6
-    assert abs(s["S"] - 1.752156) < 1e-6
+    assert abs(s["p"] - g["p_star"]) < 1e-6
+    assert abs(s["u"] - g["u_star"]) < 1e-6
+    assert abs(s["rsl"] - g["rho_star_L"]) < 1e-6
+    assert abs(s["rsr"] - g["rho_star_R"]) < 1e-6
+    assert abs(s["S"] - g["shock_speed"]) < 1e-6
+    assert abs(0.5 + 0.2 * s["head"] - g["x_head"]) < 1e-6
+    assert abs(0.5 + 0.2 * s["tail"] - g["x_tail"]) < 1e-6
+    assert abs(0.5 + 0.2 * s["u"] - g["x_contact"]) < 1e-6
+    assert abs(0.5 + 0.2 * s["S"] - g["x_shock"]) < 1e-6
 
 
 @pytest.mark.parametrize("scheme", [W.WENOZ5, W.TENO5])
@@ -212,6 +226,44 @@ def test_p6_central_stencils_exact_to_degree_4(periodic):
             assert abs(O.d2(f, i, periodic, h, pad=pad) - e2) < 1e-11 * scale, (deg, i)
     # the printed eq. (28) is -f' (Q1): the corrected sign gives +1 on f = x
     assert O.d1(x, 4, periodic, h, pad=pad) == pytest.approx(1.0, abs=1e-13)
+
+
+def test_p6_printed_coefficients_of_eq_28_to_35():
+    """Unit impulses through the oracle's difference operators reproduce the coefficients the paper
+    prints (tests/golden/central_closure_coefficients.txt, PAPER.md:200-228); eq. (34)-(35) mirrored
+    at the far end (same coefficients, reversed order: DESIGN.md / SURVEY.md O3)."""
+    n, h = 11, 0.25
+    rows = {}
+    for line in (GOLDEN / "central_closure_coefficients.txt").read_text().splitlines():
+        if line.strip() and not line.startswith("#"):
+            name, _cite, _node, first, coef = [t.strip() for t in line.split("|")]
+            rows[name] = (int(first), [float(c) for c in coef.split()])
+    node_of = {"interior": 5, "node0": 0, "node1": 1, "nodeN-2": n - 2, "nodeN-1": n - 1}
+    for name, (first, coef) in rows.items():
+        kind, where = name.split("_", 1)
+        i = node_of[where]
+        op, scale = (O.d1, 12.0 * h) if kind == "d1" else (O.d2, 12.0 * h * h)
+        got = []
+        for m in range(n):
+            e = np.zeros(n)
+            e[m] = 1.0
+            got.append(op(e, i, False, h) * scale)
+        want = np.zeros(n)
+        want[i + first:i + first + 5] = coef
+        assert np.allclose(got, want, atol=1e-12), (name, got, want)
+    # mirrored second-derivative closures at N-1, N-2
+    for where, src in (("nodeN-1", "d2_node0"), ("nodeN-2", "d2_node1")):
+        i = node_of[where]
+        first, coef = rows[src]
+        want = np.zeros(n)
+        lo = (n - 1) - (node_of[src.split("_", 1)[1]] + first + 4)
+        want[lo:lo + 5] = coef[::-1]
+        got = []
+        for m in range(n):
+            e = np.zeros(n)
+            e[m] = 1.0
+            got.append(O.d2(e, i, False, h) * 12.0 * h * h)
+        assert np.allclose(got, want, atol=1e-12), (where, got, want)
 
 
 def test_p6_closures_do_not_read_halos():
