@@ -192,6 +192,7 @@ int osbli_init(const osbli_params *p, void *d_workspace, size_t workspace_bytes,
   P.cq = p->visc != OSBLI_VISC_NONE ? 1.0 / ((p->gamma - 1.0) * p->Minf * p->Minf * p->Pr * p->Re) : 0.0;
   P.scheme = p->scheme; P.visc = p->visc;
   P.ct = p->teno_ct; P.eps = p->eps; P.suth = p->suth_ratio;
+  P.teno_kfast = (std::pow(3.0 * p->teno_ct, -1.0 / 6.0) - 1.0) * (1.0 - 1e-6);
   P.dirichlet = p->dirichlet;
   if (p->metrics) {
     for (int k = 0; k < 3; ++k) {

@@ -19,8 +19,14 @@ namespace osbli {
 // ---------------------------------------------------------------------------------------------
 // y / z sweeps
 // ---------------------------------------------------------------------------------------------
+#ifndef OSBLI_YZ_MINB
+#define OSBLI_YZ_MINB 1
+#endif
+#ifndef OSBLI_X_MINB
+#define OSBLI_X_MINB 1
+#endif
 template <int DIR, int SCHEME, bool CURV, bool ACCUM>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, CURV ? 1 : OSBLI_YZ_MINB)
 sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
                 int chunk) {
   static_assert(DIR == 1 || DIR == 2, "x has its own kernel");
@@ -34,7 +40,7 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
   const long long st = (DIR == 1) ? Ly.sy : Ly.sz;
   const long long line0 = (DIR == 1) ? Ly.at(i, 0, t) : Ly.at(i, t, 0);   // node 0 of this line
   const long long sv = Ly.sv;
-  const double eps12 = 48.0 * P.eps;
+  const RecPar rp = make_recpar(P);
   const double inv_d = P.inv_delta[DIR];
 
   Pt<CURV> w[6];
@@ -86,8 +92,8 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
     }
     const RoeSide rr = roe_side<CURV>(w[3], rsq[0]);
     double f[5];
-    if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, rl, rr, eps12, f);
-    else interface_flux<DIR, SCHEME>(P, w, rl, rr, eps12, f);
+    if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, rl, rr, rp, f);
+    else interface_flux<DIR, SCHEME>(P, w, rl, rr, rp, f);
     rl = rr;
     if (q >= s0) {
       const long long o = line0 + (long long)q * st;
@@ -114,7 +120,7 @@ template <bool CURV> struct XSmem {
 };
 
 template <int SCHEME, bool CURV>
-__global__ void __launch_bounds__(kXWarps * 32)
+__global__ void __launch_bounds__(kXWarps * 32, CURV ? 1 : OSBLI_X_MINB)
 sweep_x_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
                int chunk, int accumulate) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -131,7 +137,7 @@ sweep_x_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q
   const int nx = Ly.n[0];
   const int s0 = blockIdx.y * chunk;                             // chunk is a multiple of kXT
   const int s1 = min(s0 + chunk, nx);
-  const double eps12 = 48.0 * P.eps;
+  const RecPar rp = make_recpar(P);
   const double inv_d = P.inv_delta[0];
 
   // cooperative tile load: 32 rows x 8 points, each instruction moves 4 rows of 64 bytes
@@ -208,8 +214,8 @@ sweep_x_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q
     if (q < s0 - 1) continue;
     const RoeSide rr = roe_side<CURV>(w[3], rsq[0]);
     double f[5];
-    if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, rl, rr, eps12, f);
-    else interface_flux<0, SCHEME>(P, w, rl, rr, eps12, f);
+    if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, rl, rr, rp, f);
+    else interface_flux<0, SCHEME>(P, w, rl, rr, rp, f);
     rl = rr;
     if (q >= s0) {
       double sc = inv_d;
