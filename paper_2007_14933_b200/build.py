@@ -37,6 +37,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         return LIB
     objs = []
     flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"]
+    flags += os.environ.get("OSBLI_NVCC_EXTRA", "").split()      # tuning experiments (-D... macros)
     for src in SOURCES:
         obj = CSRC / (src[:-3] + ".o")
         cmd = [nvcc(), *flags, "-c", str(CSRC / src), "-o", str(obj)]
