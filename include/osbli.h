@@ -90,8 +90,9 @@ typedef struct {
  * OSBLI_EINVAL if a dimension is < 1 or an active one is < 5. */
 int osbli_get_layout(const osbli_params *p, osbli_layout *out);
 
-/* Bytes of device workspace osbli_init needs: one residual state R (used by osbli_rk3_step) and,
- * when visc != NONE, the staged primitive fields u, v, w, T (and mu for Sutherland). */
+/* Bytes of device workspace osbli_init needs: three states (the residual R and the two
+ * intermediate states Q2, Q3 of osbli_rk3_step, see there) and, when visc != NONE, the staged
+ * primitive fields u, v, w, T (and mu for Sutherland). */
 int osbli_workspace_bytes(const osbli_params *p, size_t *out);
 
 /* Validates *p, records it and the workspace (DEVICE pointer, 256-byte aligned, >= the size
@@ -117,7 +118,11 @@ int osbli_rhs(osbli_handle h, const double *d_Q, double *d_R, void *cuda_stream)
 
 /* One low-storage RK3 step, eq. (36)-(38): for s in 0..2 { bc(Q); R = rhs(Q);
  * Qtmp = A_s Qtmp + dt R; Q += B_s Qtmp } then bc(Q).  d_Qtmp is the dU accumulator of eq. (36);
- * it is overwritten (A_0 = 0) and need not be initialised.  R lives in the workspace. */
+ * it is overwritten (A_0 = 0) and need not be initialised.  R lives in the workspace.
+ * With two or more active directions the update is done by the last sweep kernel of each stage
+ * (no separate pass over R), which cannot update in place: the state moves d_Q -> Q2 -> Q3 ->
+ * d_Q through two workspace states; the result is in d_Q with its halos filled.  The viscous
+ * terms are added in front of the last sweep.  1-D problems update d_Q in place. */
 int osbli_rk3_step(osbli_handle h, double *d_Q, double *d_Qtmp, double dt, void *cuda_stream);
 
 /* End-to-end convenience with HOST buffers: copies h_Q (host, padded layout, total_doubles

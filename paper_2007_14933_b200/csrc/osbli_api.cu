@@ -16,6 +16,7 @@ struct ProfiledLaunch { int cls; cudaEvent_t t0, t1; };
 struct osbli_ctx {
   DevParams P;
   double *R;          // residual state in the workspace (used by osbli_rk3_step)
+  double *Q2, *Q3;    // two more states in the workspace: targets of the fused sweep + stage update
   double *prim;       // staged u, v, w, T (, mu) fields in the workspace
   int64_t launches;
   bool profiling;
@@ -108,26 +109,50 @@ int do_bc(osbli_ctx *h, double *Q, cudaStream_t st) {
   return OSBLI_OK;
 }
 
-int do_rhs(osbli_ctx *h, const double *Q, double *R, cudaStream_t st) {
+// Residual of one stage.  Order: every sweep but the last, the viscous terms, the last sweep.
+// With rk != nullptr the last sweep (y or z) also does the stage update (RkArgs) and R is left
+// without the last direction's flux difference.
+int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStream_t st) {
   const DevParams &P = h->P;
   const bool fast_visc = viscous_fast_path(P);
   if (P.visc != OSBLI_VISC_NONE && !fast_visc) OSBLI_LAUNCH(h, OSBLI_K_PRIM, st, launch_primitives(P, Q, h->prim, st));
+  int last = 0;
+  for (int d = 0; d < 3; ++d)
+    if (P.L.n[d] > 1) last = d;
   int accumulate = 0;
   for (int d = 0; d < 3; ++d) {
     if (P.L.n[d] <= 1) continue;
-    OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep(P, d, Q, R, accumulate, st));
+    if (d == last && last > 0) {                                    // viscous terms go in front of the last sweep
+      if (fast_visc) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous_fast(P, Q, R, st));
+      else if (P.visc != OSBLI_VISC_NONE) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, accumulate, st));
+    }
+    OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep(P, d, Q, R, accumulate, d == last ? rk : nullptr, st));
     accumulate = 1;
   }
-  if (fast_visc) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous_fast(P, Q, R, st));
-  else if (P.visc != OSBLI_VISC_NONE) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, accumulate, st));
+  if (last == 0 && P.visc != OSBLI_VISC_NONE)                       // 1-D: the x sweep, then the viscous terms
+    OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, accumulate, st));
   return OSBLI_OK;
 }
 
+// One low-storage RK3 step, eq. (36)-(38).  With two or more active directions the update is fused
+// into the last sweep of every stage, which cannot update in place, so the state moves
+// Q -> Q2 -> Q3 -> Q through two workspace states; 1-D problems use the separate in-place update
+// kernel.  The result is in Q either way.
 int do_step(osbli_ctx *h, double *Q, double *Qtmp, double dt, cudaStream_t st) {
+  const bool fuse = h->P.L.n[1] > 1 || h->P.L.n[2] > 1;
+  double *const chain[4] = {Q, h->Q2, h->Q3, Q};
   for (int s = 0; s < 3; ++s) {
-    if (int rc = do_bc(h, Q, st)) return rc;
-    if (int rc = do_rhs(h, Q, h->R, st)) return rc;
-    OSBLI_LAUNCH(h, OSBLI_K_RK, st, launch_rk_update(h->P, s, dt, Q, Qtmp, h->R, st));
+    if (fuse) {
+      if (int rc = do_bc(h, chain[s], st)) return rc;
+      RkArgs rk;
+      rk_coefficients(s, &rk.A, &rk.B);
+      rk.dt = dt; rk.Qtmp = Qtmp; rk.Qout = chain[s + 1]; rk.first = (s == 0);
+      if (int rc = do_rhs(h, chain[s], h->R, &rk, st)) return rc;
+    } else {
+      if (int rc = do_bc(h, Q, st)) return rc;
+      if (int rc = do_rhs(h, Q, h->R, nullptr, st)) return rc;
+      OSBLI_LAUNCH(h, OSBLI_K_RK, st, launch_rk_update(h->P, s, dt, Q, Qtmp, h->R, st));
+    }
   }
   return do_bc(h, Q, st);
 }
@@ -154,7 +179,7 @@ int osbli_workspace_bytes(const osbli_params *p, size_t *out) {
   Layout L;
   if (int rc = make_layout(p, &L)) return rc;
   if (p->visc < OSBLI_VISC_NONE || p->visc > OSBLI_VISC_SUTHERLAND) return OSBLI_EINVAL;
-  *out = (size_t)(5 + nprim(p)) * (size_t)L.sv * sizeof(double);
+  *out = (size_t)(15 + nprim(p)) * (size_t)L.sv * sizeof(double);   // R, Q2, Q3, staged primitives
   return OSBLI_OK;
 }
 
@@ -204,7 +229,9 @@ int osbli_init(const osbli_params *p, void *d_workspace, size_t workspace_bytes,
   h->prof = new (std::nothrow) std::vector<ProfiledLaunch>();
   if (!h->prof) { delete h; return OSBLI_EINVAL; }
   h->R = static_cast<double *>(d_workspace);
-  h->prim = h->R + 5 * P.L.sv;
+  h->Q2 = h->R + 5 * P.L.sv;
+  h->Q3 = h->Q2 + 5 * P.L.sv;
+  h->prim = h->Q3 + 5 * P.L.sv;
   *out = h;
   return OSBLI_OK;
 }
@@ -216,7 +243,7 @@ int osbli_bc(osbli_handle h, double *d_Q, void *cuda_stream) {
 
 int osbli_rhs(osbli_handle h, const double *d_Q, double *d_R, void *cuda_stream) {
   if (!h || !d_Q || !d_R || d_Q == d_R) return OSBLI_EINVAL;
-  return do_rhs(h, d_Q, d_R, as_stream(cuda_stream));
+  return do_rhs(h, d_Q, d_R, nullptr, as_stream(cuda_stream));
 }
 
 int osbli_rk3_step(osbli_handle h, double *d_Q, double *d_Qtmp, double dt, void *cuda_stream) {

@@ -132,10 +132,16 @@ rk_update_kernel(const __grid_constant__ DevParams P, double A, double B, double
   }
 }
 
+void rk_coefficients(int stage, double *A, double *B) {
+  const double a[3] = {0.0, -5.0 / 9.0, -153.0 / 128.0};
+  const double b[3] = {1.0 / 3.0, 15.0 / 16.0, 8.0 / 15.0};
+  *A = a[stage]; *B = b[stage];
+}
+
 cudaError_t launch_rk_update(const DevParams &P, int stage, double dt, double *Q, double *Qtmp, const double *R,
                              cudaStream_t st) {
-  const double A[3] = {0.0, -5.0 / 9.0, -153.0 / 128.0};
-  const double B[3] = {1.0 / 3.0, 15.0 / 16.0, 8.0 / 15.0};
+  double A[3], B[3];
+  for (int s = 0; s < 3; ++s) rk_coefficients(s, &A[s], &B[s]);
   const Layout &L = P.L;
   const int pairs = (L.n[0] + 1) / 2;
   dim3 grid((pairs + 127) / 128, L.n[1], L.n[2]);

@@ -4,8 +4,15 @@
 
 namespace osbli {
 
-// R (-)= flux difference of the characteristic reconstruction along `dir` (osbli_sweep.cu)
-cudaError_t launch_sweep(const DevParams &P, int dir, const double *Q, double *R, int accumulate, cudaStream_t st);
+// Runge-Kutta stage update fused into the last sweep of a stage (eq. (36)-(37)):
+// dU = A dU + dt R, Qout = Q + B dU; `first` = stage 1 (A = 0, dU not read).  Qout != Q.
+struct RkArgs { double A, B, dt; double *Qtmp, *Qout; int first; };
+void rk_coefficients(int stage, double *A, double *B);
+
+// R (-)= flux difference of the characteristic reconstruction along `dir` (osbli_sweep.cu).
+// rk != nullptr (dir 1 or 2, accumulate = 1 only): R is read but not written, the stage update is done instead.
+cudaError_t launch_sweep(const DevParams &P, int dir, const double *Q, double *R, int accumulate, const RkArgs *rk,
+                         cudaStream_t st);
 
 // staged primitive fields u, v, w, T (, mu) on the halo-extended grid, then R += viscous terms (osbli_visc.cu)
 cudaError_t launch_primitives(const DevParams &P, const double *Q, double *prim, cudaStream_t st);

@@ -22,13 +22,21 @@ namespace osbli {
 #ifndef OSBLI_YZ_MINB
 #define OSBLI_YZ_MINB 1
 #endif
+__device__ __forceinline__ void prefetch_l1(const double *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 #ifndef OSBLI_X_MINB
 #define OSBLI_X_MINB 1
 #endif
-template <int DIR, int SCHEME, bool CURV, bool ACCUM>
+// RK = 0: R (-)= flux difference.  RK = 1 / 2: this is the last kernel of the stage and also does
+// the low-storage Runge-Kutta update eq. (36)-(37) of its nodes (1: first stage, A_0 = 0, dU is not
+// read): with R_in the residual accumulated by the earlier kernels of the stage,
+//   dU = A dU + dt (R_in - (f^_{q+1/2} - f^_{q-1/2})/Delta),   Qout = Q + B dU,
+// evaluated as (A dU + dt R_in) + (dt/Delta)(f^_{q-1/2} - f^_{q+1/2}) so that one value per variable
+// waits in registers for the flux.  Q of node q is window slot 2; Qout must not alias Q (other
+// blocks still read Q next to the chunk boundaries).  The final residual is not written anywhere.
+template <int DIR, int SCHEME, bool CURV, bool ACCUM, int RK>
 __global__ void __launch_bounds__(128, CURV ? 1 : OSBLI_YZ_MINB)
 sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
-                int chunk) {
+                int chunk, const RkArgs rk) {
   static_assert(DIR == 1 || DIR == 2, "x has its own kernel");
   const Layout &Ly = P.L;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -81,13 +89,19 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
     rsq[0] = rsq[1]; rsq[1] = rsq[2];
     make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], w[5], rsq[2]);
     if (q + 1 < s1) load(q + 4, qn, Kn);         // node (q+1)+3, used by the next interface
-    // R of node q is read now and consumed after the flux: its latency hides behind ~1000 DFMAs
+    // R of node q is read now and consumed after the flux: its latency hides behind ~600 DFMAs.
+    // dU of the fused update is only prefetched into L1 here and loaded after the flux (holding it
+    // in registers as well costs more than the late L1 hit: measured).
     double rold[5] = {0, 0, 0, 0, 0};
-    if constexpr (ACCUM) {
-      if (q >= s0) {
-        const long long o = line0 + (long long)q * st;
+    if (q >= s0) {
+      const long long o = line0 + (long long)q * st;
+      if constexpr (ACCUM) {
 #pragma unroll
         for (int c = 0; c < 5; ++c) rold[c] = R[c * sv + o];
+      }
+      if constexpr (RK == 2) {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) prefetch_l1(rk.Qtmp + c * sv + o);
       }
     }
     const RoeSide rr = roe_side<CURV>(w[3], rsq[0]);
@@ -99,8 +113,31 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
       const long long o = line0 + (long long)q * st;
       double sc = inv_d;
       if constexpr (CURV) sc = 1.0 / __ldg(P.detJ + o);
+      if constexpr (RK != 0) {
+        double dold[5] = {0, 0, 0, 0, 0};
+        if constexpr (RK == 2) {
 #pragma unroll
-      for (int c = 0; c < 5; ++c) R[c * sv + o] = fma(prev[c] - f[c], sc, rold[c]);
+          for (int c = 0; c < 5; ++c) dold[c] = rk.Qtmp[c * sv + o];
+        }
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {
+          rold[c] *= rk.dt;
+          if constexpr (RK == 2) rold[c] = fma(rk.A, dold[c], rold[c]);
+        }
+      }
+      if constexpr (RK == 0) {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) R[c * sv + o] = fma(prev[c] - f[c], sc, rold[c]);
+      } else {
+        const double qc[5] = {w[2].r, w[2].m[0], w[2].m[1], w[2].m[2], w[2].E};   // slot 2 = node q
+        sc *= rk.dt;
+#pragma unroll
+        for (int c = 0; c < 5; ++c) {
+          const double d = fma(prev[c] - f[c], sc, rold[c]);
+          rk.Qtmp[c * sv + o] = d;
+          rk.Qout[c * sv + o] = fma(rk.B, d, qc[c]);
+        }
+      }
     }
 #pragma unroll
     for (int c = 0; c < 5; ++c) prev[c] = f[c];
@@ -257,26 +294,34 @@ static cudaError_t launch_x(const DevParams &P, const double *Q, double *R, int 
 }
 
 template <int DIR, int SCHEME, bool CURV>
-static cudaError_t launch_yz(const DevParams &P, const double *Q, double *R, int accumulate, cudaStream_t st) {
+static cudaError_t launch_yz(const DevParams &P, const double *Q, double *R, int accumulate, const RkArgs *rk,
+                             cudaStream_t st) {
   const int nx = P.L.n[0];
   const int n = P.L.n[DIR];
   const int nt = (DIR == 1) ? P.L.n[2] : P.L.n[1];
   const int bx = nx >= 128 ? 128 : (nx > 64 ? 128 : (nx > 32 ? 64 : 32));
   int chunk = n > 64 ? 32 : n;
   dim3 grid((nx + bx - 1) / bx, nt, (n + chunk - 1) / chunk);
-  if (accumulate) sweep_yz_kernel<DIR, SCHEME, CURV, true><<<grid, bx, 0, st>>>(P, Q, R, chunk);
-  else sweep_yz_kernel<DIR, SCHEME, CURV, false><<<grid, bx, 0, st>>>(P, Q, R, chunk);
+  const RkArgs none = {0.0, 0.0, 0.0, nullptr, nullptr};
+  if (rk) {
+    if (!accumulate) return cudaErrorInvalidValue;              // the fused update is never the first kernel
+    if (rk->first) sweep_yz_kernel<DIR, SCHEME, CURV, true, 1><<<grid, bx, 0, st>>>(P, Q, R, chunk, *rk);
+    else sweep_yz_kernel<DIR, SCHEME, CURV, true, 2><<<grid, bx, 0, st>>>(P, Q, R, chunk, *rk);
+  } else if (accumulate) sweep_yz_kernel<DIR, SCHEME, CURV, true, 0><<<grid, bx, 0, st>>>(P, Q, R, chunk, none);
+  else sweep_yz_kernel<DIR, SCHEME, CURV, false, 0><<<grid, bx, 0, st>>>(P, Q, R, chunk, none);
   return cudaGetLastError();
 }
 
-cudaError_t launch_sweep(const DevParams &P, int dir, const double *Q, double *R, int accumulate, cudaStream_t st) {
+cudaError_t launch_sweep(const DevParams &P, int dir, const double *Q, double *R, int accumulate, const RkArgs *rk,
+                         cudaStream_t st) {
   const bool curv = P.curvilinear != 0;
   const int sch = P.scheme;
+  if (rk && dir == 0) return cudaErrorInvalidValue;             // only the y / z sweeps carry the fused update
 #define OSBLI_DISPATCH(SCH, CRV)                                              \
   if (sch == SCH && curv == CRV) {                                            \
     if (dir == 0) return launch_x<SCH, CRV>(P, Q, R, accumulate, st);         \
-    if (dir == 1) return launch_yz<1, SCH, CRV>(P, Q, R, accumulate, st);     \
-    return launch_yz<2, SCH, CRV>(P, Q, R, accumulate, st);                   \
+    if (dir == 1) return launch_yz<1, SCH, CRV>(P, Q, R, accumulate, rk, st); \
+    return launch_yz<2, SCH, CRV>(P, Q, R, accumulate, rk, st);               \
   }
   OSBLI_DISPATCH(0, false)
   OSBLI_DISPATCH(1, false)
