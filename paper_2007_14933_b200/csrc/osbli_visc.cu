@@ -253,6 +253,9 @@ cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *pr
 // derivatives and the in-plane stencils read shared memory (84 LDS.64 per node).  One barrier per
 // plane.  R is read at the top of a step and written at its end.
 // =============================================================================================
+#ifndef OSBLI_VCHUNK
+#define OSBLI_VCHUNK 32
+#endif
 constexpr int kVX = 32, kVY = 8, kVH = 2;
 constexpr int kVPX = kVX + 2 * kVH, kVPY = kVY + 2 * kVH;        // 36 x 12 plane tile
 constexpr int kVRing = 4;
@@ -320,15 +323,22 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
 #pragma unroll
   for (int m = 0; m < 5; ++m) uw[m] = vw[m] = ww[m] = Tw[m] = uxw[m] = vyw[m] = wxw[m] = wyw[m] = 0.0;
 
+  // Software pipeline, one barrier per plane: during step k (node k is finished) plane k+3 is
+  // staged into the slot plane k-1 has just left, plane k+4 is fetched into registers, plane k+2
+  // (staged one step earlier) enters the register windows and plane k is the centre of the
+  // in-plane stencils -- so staging, global loads and the stencil arithmetic of a step are
+  // independent of each other and the barrier closes the step.
   double qn[2][5];
   fetch(z0 - 2, qn);
+  stage(z0 - 2, qn);
+  fetch(z0 - 1, qn);
+  __syncthreads();
   const int X = tx + kVH, Y = ty + kVH;
 
-  for (int k = z0 - 4; k < z1; ++k) {            // step k: plane k+2 enters, node k is finished
-    const int pe = k + 2;
-    const bool entering = pe >= z0 - 2;
-    if (entering) stage(pe, qn);
-    if (pe + 1 >= z0 - 2 && pe + 1 < z1 + 2) fetch(pe + 1, qn);
+  for (int k = z0 - 4; k < z1; ++k) {
+    if (k > z0 - 4) __syncthreads();
+    if (k + 3 < z1 + 2) stage(k + 3, qn);
+    if (k + 4 < z1 + 2) fetch(k + 4, qn);
     double rold[4] = {0, 0, 0, 0};
     long long at = 0;
     if (k >= z0 && inside) {
@@ -336,14 +346,13 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
 #pragma unroll
       for (int c = 0; c < 4; ++c) rold[c] = R[(c + 1) * sv + at];
     }
-    __syncthreads();
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
       uw[m] = uw[m + 1]; vw[m] = vw[m + 1]; ww[m] = ww[m + 1]; Tw[m] = Tw[m + 1];
       uxw[m] = uxw[m + 1]; vyw[m] = vyw[m + 1]; wxw[m] = wxw[m + 1]; wyw[m] = wyw[m + 1];
     }
-    if (entering) {
-      const double (*F)[kVPY][kVPX] = S.f[(pe + 8) & (kVRing - 1)];
+    {
+      const double (*F)[kVPY][kVPX] = S.f[(k + 2 + 8) & (kVRing - 1)];      // plane k+2
       uw[4] = F[0][Y][X]; vw[4] = F[1][Y][X]; ww[4] = F[2][Y][X]; Tw[4] = F[3][Y][X];
       uxw[4] = d1(F[0][Y][X - 2], F[0][Y][X - 1], F[0][Y][X + 1], F[0][Y][X + 2], cx);
       wxw[4] = d1(F[2][Y][X - 2], F[2][Y][X - 1], F[2][Y][X + 1], F[2][Y][X + 2], cx);
@@ -422,7 +431,7 @@ bool viscous_fast_path(const DevParams &P) {
 
 cudaError_t launch_viscous_fast(const DevParams &P, const double *Q, double *R, cudaStream_t st) {
   const Layout &L = P.L;
-  const int chunk = L.n[2] > 64 ? 64 : L.n[2];
+  const int chunk = L.n[2] > OSBLI_VCHUNK ? OSBLI_VCHUNK : L.n[2];
   dim3 grid((L.n[0] + kVX - 1) / kVX, (L.n[1] + kVY - 1) / kVY, (L.n[2] + chunk - 1) / chunk);
   static bool attr_done = false;
   if (!attr_done) {
