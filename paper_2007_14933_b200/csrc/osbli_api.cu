@@ -140,13 +140,17 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
 // kernel.  The result is in Q either way.
 int do_step(osbli_ctx *h, double *Q, double *Qtmp, double dt, cudaStream_t st) {
   const bool fuse = h->P.L.n[1] > 1 || h->P.L.n[2] > 1;
+  bool wrap = fuse;                  // every active direction periodic: the fused update fills the halos itself
+  for (int d = 0; d < 3; ++d)
+    if (h->P.L.n[d] > 1 && !h->P.periodic[d]) wrap = false;
   double *const chain[4] = {Q, h->Q2, h->Q3, Q};
   for (int s = 0; s < 3; ++s) {
     if (fuse) {
-      if (int rc = do_bc(h, chain[s], st)) return rc;
+      if (s == 0 || !wrap)
+        if (int rc = do_bc(h, chain[s], st)) return rc;
       RkArgs rk;
       rk_coefficients(s, &rk.A, &rk.B);
-      rk.dt = dt; rk.Qtmp = Qtmp; rk.Qout = chain[s + 1]; rk.first = (s == 0);
+      rk.dt = dt; rk.Qtmp = Qtmp; rk.Qout = chain[s + 1]; rk.first = (s == 0); rk.wrap = wrap ? 1 : 0;
       if (int rc = do_rhs(h, chain[s], h->R, &rk, st)) return rc;
     } else {
       if (int rc = do_bc(h, Q, st)) return rc;
@@ -154,7 +158,7 @@ int do_step(osbli_ctx *h, double *Q, double *Qtmp, double dt, cudaStream_t st) {
       OSBLI_LAUNCH(h, OSBLI_K_RK, st, launch_rk_update(h->P, s, dt, Q, Qtmp, h->R, st));
     }
   }
-  return do_bc(h, Q, st);
+  return wrap ? OSBLI_OK : do_bc(h, Q, st);
 }
 
 }  // namespace

@@ -6,7 +6,9 @@ namespace osbli {
 
 // Runge-Kutta stage update fused into the last sweep of a stage (eq. (36)-(37)):
 // dU = A dU + dt R, Qout = Q + B dU; `first` = stage 1 (A = 0, dU not read).  Qout != Q.
-struct RkArgs { double A, B, dt; double *Qtmp, *Qout; int first; };
+// wrap != 0 (all active directions periodic): the periodic images of the boundary-near nodes are
+// written into the halos of Qout as well, which replaces the halo fill of the next stage.
+struct RkArgs { double A, B, dt; double *Qtmp, *Qout; int first, wrap; };
 void rk_coefficients(int stage, double *A, double *B);
 
 // R (-)= flux difference of the characteristic reconstruction along `dir` (osbli_sweep.cu).

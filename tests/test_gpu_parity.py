@@ -172,6 +172,39 @@ def test_steps_curvilinear_walls():
     run_steps_case("wavy_box_5", case, 5, 1e-9, parity.l1_rel)
 
 
+def _periodic_box(n, M=0.4, Re=100.0, scheme=W.TENO5, visc=W.VISC_CONST, bc=None, dt=2e-3):
+    """Smooth periodic field on an n[0] x n[1] x n[2] box (n_d = 1: inactive direction)."""
+    i, j, k = W.padded_index_grids(n)
+    x, y, z = 2 * np.pi * i / n[0], 2 * np.pi * j / n[1], 2 * np.pi * k / n[2]
+    g = 1.4
+    u = np.sin(x) * np.cos(y) * np.cos(z)
+    v = -np.cos(x) * np.sin(y) * np.cos(z)
+    w = (0.3 * np.sin(x + y) * np.sin(z)) if n[2] > 1 else 0.0 * x
+    p = 1.0 / (g * M * M) + (np.cos(2 * x) + np.cos(2 * y)) * (np.cos(2 * z) + 2.0) / 16.0
+    rho = 1.0 + 0.2 * np.sin(x + 2 * y - z)
+    per = (W.BC_PERIODIC, W.BC_PERIODIC)
+    return W.Case(name="pbox", n=n, Q0=np.ascontiguousarray(W.conservative(rho, u, v, w, p, g)), dt=dt, nsteps=3,
+                  delta=tuple(2 * np.pi / v_ for v_ in n), gamma=g, Re=Re, Pr=0.71, Minf=M, scheme=scheme, visc=visc,
+                  bc=bc if bc is not None else (per, per, per))
+
+
+def test_steps_fused_update_ragged_periodic():
+    """The stage update fused into the last sweep, with the periodic images of boundary-near nodes
+    written straight into the halos (no halo-fill pass between stages): ragged sizes spanning
+    several chunks, the smallest legal size (n = 5: node 2 has an image on both sides), a 2-D
+    problem (last sweep = y).  run_steps_case compares the halos of the final state as well."""
+    run_steps_case("pbox_70x37x35", _periodic_box((70, 37, 35)), 3, 1e-9, parity.q28)
+    run_steps_case("pbox_130x5x6", _periodic_box((130, 5, 6), dt=5e-4), 3, 1e-9, parity.q28)
+    run_steps_case("pbox2d_40x33", _periodic_box((40, 33, 1)), 3, 1e-9, parity.q28)
+    run_steps_case("pbox_wenoz_euler", _periodic_box((33, 34, 9), scheme=W.WENOZ5, visc=W.VISC_NONE), 3, 1e-9, parity.q28)
+
+
+def test_steps_fused_update_mixed_boundaries():
+    """Periodic in x and z, extrapolation in y: the fused update runs, the halo fill stays a separate pass."""
+    per, ex = (W.BC_PERIODIC, W.BC_PERIODIC), (W.BC_EXTRAP0, W.BC_EXTRAP0)
+    run_steps_case("pbox_mixed_bc", _periodic_box((36, 20, 10), bc=(per, ex, per), dt=1e-3), 3, 1e-9, parity.q28)
+
+
 def test_advance_host_matches_device_steps():
     case = W.tgv(32)
     sol = parity.make_solver(case)
