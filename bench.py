@@ -105,12 +105,13 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0}, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic_bytes():
-    """dram read+write bytes per launch of the dominant kernel from the committed ncu capture, if any."""
+def ncu_traffic_bytes(kernel):
+    """dram read+write bytes per launch of `kernel` (sweep_x / sweep_y / sweep_z) from the committed
+    ncu capture (profiles/dominant_kernel_traffic.txt), if it has one."""
     p = ROOT / "profiles" / "dominant_kernel_traffic.txt"
     try:
         for line in p.read_text().splitlines():
-            if line.startswith("traffic_bytes_per_launch="):
+            if line.startswith(f"traffic_bytes_per_launch[{kernel}]="):
                 return float(line.split("=", 1)[1])
     except Exception:
         pass
@@ -266,7 +267,10 @@ def run_ours(args):
     dom = max(("sweep_x", "sweep_y", "sweep_z"), key=lambda k: prof[k][0])
     dom_ms, dom_cnt = prof[dom]
     dom_avg_s = dom_ms * 1e-3 / max(dom_cnt, 1)
-    flop_launch = FLOP_SWEEP[case.scheme] * npts
+    # the stage update is fused into the last sweep (z) when no separate update kernel ran
+    fused = prof["rk_update"][1] == 0
+    flop_point = FLOP_SWEEP[case.scheme] + (FLOP_RK if (fused and dom == "sweep_z") else 0)
+    flop_launch = flop_point * npts
     achieved = flop_launch / dom_avg_s * 1e-12
     peaks, peak_src = measured_peaks()
     total_prof_ms = sum(v[0] for v in prof.values())
@@ -274,9 +278,10 @@ def run_ours(args):
     roofline = {
         "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
         "frac": achieved / peak_tflops if peak_tflops > 0 else None,
-        "traffic": ncu_traffic_bytes(),
+        "traffic": ncu_traffic_bytes(dom),
         "peak_source": "fp64 DFMA micro-benchmark run in this process (osbli_measure_fp64_peak); nominal 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2",
-        "algorithmic_flop_per_point": FLOP_SWEEP[case.scheme],
+        "algorithmic_flop_per_point": flop_point,
+        "fused_stage_update": fused,
         "avg_launch_ms": dom_avg_s * 1e3,
         "whole_step_useful_flop_frac": step_flop * value / world * 1e-12 / peak_tflops if peak_tflops > 0 else None,
         "kernel_share_of_step": {k: (v[0] / total_prof_ms if total_prof_ms > 0 else None) for k, v in prof.items()},
@@ -285,7 +290,8 @@ def run_ours(args):
         "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peak_src,
     }
 
-    cpu_rate, cpu_cores, cpu_dt = cpu_oracle_rate(128)
+    cpu_n = 256 if n >= 256 else n          # one RK3 step of the same field: about 10 s on 16 cores at 256^3
+    cpu_rate, cpu_cores, cpu_dt = cpu_oracle_rate(cpu_n)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -301,7 +307,7 @@ def run_ours(args):
         "gpu_launches": launches,
         "roofline": roofline,
         "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": cpu_cores, "kind": "oracle",
-                         "sample": f"1 RK3 step (3 stage evaluations) of the same TGV on 128^3 points, {cpu_dt:.1f} s"},
+                         "sample": f"1 RK3 step (3 stage evaluations) of the same TGV on {cpu_n}^3 points, {cpu_dt:.1f} s"},
     }
     print(json.dumps(line))
     sol.close()

@@ -22,7 +22,6 @@ namespace osbli {
 #ifndef OSBLI_YZ_MINB
 #define OSBLI_YZ_MINB 1
 #endif
-__device__ __forceinline__ void prefetch_l1(const double *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 #ifndef OSBLI_X_MINB
 #define OSBLI_X_MINB 1
 #endif

@@ -302,7 +302,7 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
 #pragma unroll
     for (int s = 0; s < 2; ++s)
       if (pv[s]) {
-        const double ir = 1.0 / q[s][0];
+        const double ir = fast_rcp(q[s][0]);
         const double u = q[s][1] * ir, v = q[s][2] * ir, w = q[s][3] * ir;
         const double p = P.gm1 * (q[s][4] - 0.5 * (q[s][1] * u + q[s][2] * v + q[s][3] * w));
         S.f[slot][0][pj[s]][pi[s]] = u;
