@@ -185,6 +185,133 @@ def euler_wave(N=32, scheme=WENOZ5, A=0.04, dt=5e-4, t_end=2.5, curvilinear=True
                 extra={"rho_exact": rho_exact(xi, yi, dt * nsteps), "t_end": dt * nsteps})
 
 
+# --------------------------------------------------------------------------------- C4 ------
+def sutherland(T, S=110.4 / 288.0):
+    """mu(T) of the problem statement -- used here only to build the inflow profile."""
+    return T ** 1.5 * (1.0 + S) / (T + S)
+
+
+def similarity_boundary_layer(M=2.0, Pr=0.72, gamma=1.4, S=110.4 / 288.0, eta_max=12.0, n_eta=2400):
+    """Compressible laminar similarity profile over an adiabatic wall (White, ref. [61] of the paper;
+    the SBLI inflow of PAPER.md:576-601 is such a profile):
+
+        (C f'')' + f f'' = 0,   (C g'/Pr)' + f g' + (gamma-1) M^2 C f''^2 = 0,   C = mu(g)/g,
+        f(0) = f'(0) = 0, g'(0) = 0, f'(inf) = g(inf) = 1,
+
+    f' = u/u_e, g = T/T_e, eta the Illingworth-Levy variable.  Classical RK4 on a fixed grid and Newton
+    shooting on (f''(0), g(0)).  Returns eta, f', g, Y = int_0^eta g and I = int (g - f') d eta.
+    """
+    h = eta_max / n_eta
+    gm = (gamma - 1.0) * M * M
+
+    def rhs(y):
+        f, fp, s, g, q = y
+        C = sutherland(g, S) / g
+        fpp = s / C
+        gp = Pr * q / C
+        return np.array([fp, fpp, -f * fpp, gp, -f * gp - gm * s * s / C])
+
+    def shoot(fpp0, g0, full=False):
+        C0 = sutherland(g0, S) / g0
+        y = np.array([0.0, 0.0, C0 * fpp0, g0, 0.0])
+        out = [y.copy()] if full else None
+        for _ in range(n_eta):
+            k1 = rhs(y); k2 = rhs(y + 0.5 * h * k1); k3 = rhs(y + 0.5 * h * k2); k4 = rhs(y + h * k3)
+            y = y + (h / 6.0) * (k1 + 2 * k2 + 2 * k3 + k4)
+            if full:
+                out.append(y.copy())
+        return (np.array(out) if full else None), np.array([y[1] - 1.0, y[3] - 1.0])
+
+    x = np.array([0.5, 1.0 + 0.5 * np.sqrt(Pr) * gm])          # recovery-factor guess for g(0)
+    for _ in range(30):
+        _, r = shoot(x[0], x[1])
+        if np.abs(r).max() < 1e-13:
+            break
+        J = np.empty((2, 2))
+        for c in range(2):
+            d = np.zeros(2); d[c] = 1e-7
+            _, rp = shoot(*(x + d))
+            J[:, c] = (rp - r) / 1e-7
+        x = x - np.linalg.solve(J, r)
+    sol, _ = shoot(x[0], x[1], full=True)
+    eta = h * np.arange(n_eta + 1)
+    fp, g = sol[:, 1], sol[:, 3]
+    trap = lambda a: np.concatenate([[0.0], np.cumsum(0.5 * h * (a[1:] + a[:-1]))])
+    Y = trap(g)
+    I = trap(g - fp)[-1]
+    return dict(eta=eta, fp=fp, g=g, Y=Y, I=float(I), fpp0=float(x[0]), g0=float(x[1]))
+
+
+def oblique_shock(M=2.0, beta_deg=32.58, gamma=1.4):
+    """Rankine-Hugoniot state behind an oblique shock of angle beta in a (rho, u, v, p) = (1, 1, 0, 1/(gamma M^2))
+    stream, turning the flow towards the wall (v < 0)."""
+    b = np.deg2rad(beta_deg)
+    mn2 = (M * np.sin(b)) ** 2
+    pr = 1.0 + 2.0 * gamma / (gamma + 1.0) * (mn2 - 1.0)
+    rr = (gamma + 1.0) * mn2 / ((gamma - 1.0) * mn2 + 2.0)
+    ut, un2 = np.cos(b), np.sin(b) / rr
+    return dict(rho=rr, u=ut * np.cos(b) + un2 * np.sin(b), v=-(ut * np.sin(b) - un2 * np.cos(b)),
+                p=pr / (gamma * M * M), p_ratio=pr, rho_ratio=rr)
+
+
+def sbli_slab(n=(500, 250, 8), seed=2007014933, noise=1e-4, dt=1e-3, nsteps=500, scheme=WENOZ5, x_shock=20.0):
+    """BASELINE.json config 4: quasi-2-D laminar shock / boundary-layer interaction slab on a curvilinear grid
+    (recipe: DESIGN.md "Input recipe"; set-up modelled on PAPER.md:576-601).  `n` can be reduced for quick runs:
+    the domain, the stretching and the flow stay the same."""
+    n = tuple(int(v) for v in n)
+    nx, ny, nz = n
+    gamma, M, Re, Pr, S = 1.4, 2.0, 950.0, 0.72, 110.4 / 288.0
+    Lx, Ly, dz = 300.0, 115.0, 0.6
+    i, j, k = padded_index_grids(n)
+    xi = i / (nx - 1.0) + 0.0 * j + 0.0 * k
+    et = j / (ny - 1.0) + 0.0 * i + 0.0 * k
+    x = Lx * (xi + 0.01 * np.sin(4.0 * np.pi * xi) * np.sin(4.0 * np.pi * et))
+    y = Ly * (1.0 + np.tanh(2.5 * (et - 1.0)) / np.tanh(2.5))
+    z = dz * k + 0.0 * i + 0.0 * j
+    coords = np.ascontiguousarray(np.stack([x, y, z]))
+
+    bl = similarity_boundary_layer(M, Pr, gamma, S)
+    x0 = Re / (2.0 * bl["I"] ** 2)                              # delta* = 1 at the inflow
+    ysim = np.sqrt(2.0 * x0 / Re) * bl["Y"]
+    yy = np.clip(y, 0.0, None)
+    u = np.interp(yy, ysim, bl["fp"], right=1.0)
+    T = np.interp(yy, ysim, bl["g"], right=1.0)
+    p0 = 1.0 / (gamma * M * M)
+    rho = 1.0 / T
+    clean = np.ascontiguousarray(conservative(rho, u, 0.0 * u, 0.0 * u, p0 + 0.0 * u, gamma))
+    clean = edge_pad_interior(clean, n)
+
+    # frozen boundary state: inflow profile; top boundary free stream up to x_shock, post-shock state behind
+    dirichlet = clean.copy()
+    sh = oblique_shock(M, 32.58, gamma)
+    post = conservative(sh["rho"], sh["u"], sh["v"], 0.0, sh["p"], gamma)
+    free = conservative(1.0, 1.0, 0.0, 0.0, p0, gamma)
+    h = halo_of(n)
+    top = slice(h[1] + ny - 1, None)
+    behind = (x[:, top, :] >= x_shock)
+    for c in range(5):
+        dirichlet[c][:, top, :] = np.where(behind, post[c], free[c])
+
+    # seeded density noise on interior nodes; u, v, w, p unchanged
+    ii, jj, kk = np.meshgrid(np.arange(nx), np.arange(ny), np.arange(nz), indexing="ij")
+    lin = (ii + nx * (jj + ny * kk)).astype(np.uint64)
+    r = splitmix64_unit(seed, lin).transpose(2, 1, 0)           # [nz, ny, nx]
+    core = (slice(h[2], h[2] + nz), slice(h[1], h[1] + ny), slice(h[0], h[0] + nx))
+    rho_n = rho.copy() + 0.0 * k
+    rho_n = np.broadcast_to(rho_n, clean[0].shape).copy()
+    rho_n[core] *= (1.0 + noise * r)
+    ub = np.broadcast_to(u, clean[0].shape)
+    Q0 = conservative(rho_n, ub, 0.0 * ub, 0.0 * ub, p0 + 0.0 * ub, gamma)
+    Q0 = edge_pad_interior(np.ascontiguousarray(Q0), n)
+
+    per = (BC_PERIODIC, BC_PERIODIC)
+    bc = ((BC_DIRICHLET, BC_EXTRAP0), (BC_WALL_ISOTHERMAL, BC_DIRICHLET), per if nz > 1 else (0, 0))
+    wt = ((0.0, 0.0), (bl["g0"], 0.0), (0.0, 0.0))
+    return Case(name="sbli_slab", n=n, Q0=Q0, dt=dt, nsteps=nsteps, delta=(1.0, 1.0, 1.0), coords=coords, gamma=gamma,
+                Re=Re, Pr=Pr, Minf=M, scheme=scheme, visc=VISC_SUTHERLAND, suth_ratio=S, bc=bc, wall_T=wt,
+                dirichlet=dirichlet, extra={"bl": bl, "x0": x0, "shock": sh})
+
+
 # --------------------------------------------------- small curvilinear box (parity cases) ----
 def wavy_box(n=(24, 20, 8), seed=1, bc=None, scheme=WENOZ5, visc=VISC_SUTHERLAND, M=2.0, Re=950.0, Pr=0.72,
              amp=0.05, grid_amp=0.03, wall_T=1.2, dt=1e-3, nsteps=2):

@@ -9,7 +9,10 @@ Tolerance on a single residual evaluation (per variable c, absolute):
   Q28 (den_c = ||R_c||_inf of the oracle, or the largest such norm if variable c is ~0);
 * second term: the fp64 rounding floor of the residual itself.  R is a difference of interface
   fluxes divided by the spacing, and each interface flux is a sum of characteristic contributions
-  of magnitude up to Phi_c = (|u|+a)|Q_c| (+ p for momentum, + (|u|+a) p for energy).  At low Mach
+  of magnitude up to Phi_c = (|u|+a)|Q_c| (+ (|u|+a) rho + p for momentum: the singularity-free
+  eigenvectors of DESIGN.md Q12 have unit-size entries in the momentum rows, so a momentum component
+  that is itself ~0 -- the spanwise one of the quasi-2-D slab, config 4 -- still receives
+  characteristic fluxes of size (|u|+a) rho that cancel only to rounding; + (|u|+a) p for energy).  At low Mach
   number Phi_c/Delta is ~1e5-1e6 times ||R_c||, so 1e-11 relative is below one rounding error of
   the terms being subtracted: the oracle compiled with FMA contraction (same source, same
   operation order) already differs from itself by 3.7e-11 on the 64^3 TGV, i.e. ~3 of these units
@@ -109,8 +112,11 @@ def flux_scale(case, Qi, metrics=None, points=None):
         else:
             D = [interior(case, metrics["D"][d][j]) for j in range(3)]
             geo = geo + np.sqrt(D[0] ** 2 + D[1] ** 2 + D[2] ** 2)
+    # momentum: the eigenvectors of DESIGN.md Q12 carry entries of unit size
+    # (n_z, -n_y, ...) in the momentum rows of the three theta-fields, so every momentum component
+    # receives characteristic fluxes of size (|u|+a) rho whatever its own magnitude is
     phi = [speed * np.abs(Qi[0]),
-           speed * np.abs(Qi[1]) + p, speed * np.abs(Qi[2]) + p, speed * np.abs(Qi[3]) + p,
+           speed * (np.abs(Qi[1]) + rho) + p, speed * (np.abs(Qi[2]) + rho) + p, speed * (np.abs(Qi[3]) + rho) + p,
            speed * (np.abs(Qi[4]) + p)]
     return np.array([float((f * geo).max()) for f in phi])
 
