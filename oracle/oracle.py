@@ -19,7 +19,7 @@ _SRC = _HERE / "osbli_oracle.cpp"
 _HDR = _HERE / "osbli_oracle.h"
 _LIB = _HERE / "libosbli_oracle.so"
 
-WENOZ5, TENO5 = 0, 1
+WENOZ5, TENO5, TENO6 = 0, 1, 2
 VISC_NONE, VISC_CONST, VISC_SUTHERLAND = 0, 1, 2
 BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL = 0, 1, 2, 3
 PART_INVISCID, PART_VISCOUS = 1, 2
@@ -69,6 +69,10 @@ def lib():
         L = C.CDLL(str(_LIB))
         L.oracle_reconstruct.restype = C.c_double
         L.oracle_reconstruct.argtypes = [C.c_int32] + [C.c_double] * 7 + [_dp]
+        L.oracle_reconstruct6.restype = C.c_double
+        L.oracle_reconstruct6.argtypes = [C.c_double] * 8 + [_dp]
+        L.oracle_teno6_indicators.restype = None
+        L.oracle_teno6_indicators.argtypes = [C.c_double] * 6 + [_dp]
         L.oracle_eigensystem.restype = None
         L.oracle_eigensystem.argtypes = [C.c_double, _dp, _dp, _dp, _dp, _dp, _dp]
         L.oracle_d1.restype = C.c_double
@@ -106,6 +110,18 @@ def reconstruct(scheme, a, b, c, d, e, eps=1e-16, ct=1e-6, with_margin=False):
     m = C.c_double(0.0)
     v = lib().oracle_reconstruct(scheme, a, b, c, d, e, eps, ct, C.byref(m))
     return (v, m.value) if with_margin else v
+
+
+def reconstruct6(a, b, c, d, e, f, eps=1e-16, ct=1e-6, with_margin=False):
+    m = C.c_double(0.0)
+    v = lib().oracle_reconstruct6(a, b, c, d, e, f, eps, ct, C.byref(m))
+    return (v, m.value) if with_margin else v
+
+
+def teno6_indicators(a, b, c, d, e, f):
+    out = np.zeros(5)
+    lib().oracle_teno6_indicators(a, b, c, d, e, f, _ptr(out))
+    return out
 
 
 def eigensystem(gamma, QL, QR, nhat):

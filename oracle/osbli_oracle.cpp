@@ -131,6 +131,57 @@ double reconstruct(int scheme, double a, double b, double c, double d, double e,
   return wR * qR + wC * qC + wL * qL;
 }
 
+/* ------------------------------------------------------------- TENO6 reconstruction ---- */
+/* Sixth-order TENO (OpenSBLI "has both 5th and 6th order TENO schemes"): the three
+ * 3-point candidates of eq. (14) plus a 4-point candidate on {c,d,e,f} (K - 2 = 4 stencils, r = 0..3),
+ * weights eq. (23)-(25), global indicator eq. (27): tau_6 = |beta_3 - (beta_0 + beta_2 + 4 beta_1)/6|.
+ * The paper prints neither d_r nor beta_3 for this scheme (refs [20, 21]); they follow from
+ * definitions it does give (Q32):
+ *   - q_3 = (3c + 13d - 5e + f)/12: the cubic with cell averages c,d,e,f evaluated at the interface;
+ *   - d_r: the weights for which sum_r d_r q_r is the 6th-order value (a-8b+37c+37d-8e+f)/60:
+ *     d_0 (R) = 6/20, d_1 (C) = 9/20, d_2 (L) = 1/20, d_3 = 4/20;
+ *   - beta_3: the Jiang-Shu indicator [36] of that cubic, sum_l dx^(2l-1) int (d^l p/dx^l)^2 dx over
+ *     the cell of c (re-derived symbolically in tests/test_oracle_teno6.py).
+ * beta_0 -> R, beta_1 -> C, beta_2 -> L as in eq. (17)-(19). */
+double reconstruct6(double a, double b, double c, double d, double e, double f,
+                    double eps, double ct, double *margin, double *indicators = nullptr) {
+  const double q[4] = {(2.0 * c + 5.0 * d - e) / 6.0, (-b + 5.0 * c + 2.0 * d) / 6.0,
+                       (2.0 * a - 7.0 * b + 11.0 * c) / 6.0, (3.0 * c + 13.0 * d - 5.0 * e + f) / 12.0};
+  const double dw[4] = {6.0 / 20.0, 9.0 / 20.0, 1.0 / 20.0, 4.0 / 20.0};
+  const double s0 = c - 2.0 * d + e, t0 = 3.0 * c - 4.0 * d + e;
+  const double s1 = b - 2.0 * c + d, t1 = b - d;
+  const double s2 = a - 2.0 * b + c, t2 = a - 4.0 * b + 3.0 * c;
+  double beta[4];
+  beta[0] = 13.0 / 12.0 * (s0 * s0) + 0.25 * (t0 * t0);   /* eq. (17) */
+  beta[1] = 13.0 / 12.0 * (s1 * s1) + 0.25 * (t1 * t1);   /* eq. (18) */
+  beta[2] = 13.0 / 12.0 * (s2 * s2) + 0.25 * (t2 * t2);   /* eq. (19) */
+  beta[3] = (c * (2107.0 * c - 9402.0 * d + 7042.0 * e - 1854.0 * f) +
+             d * (11003.0 * d - 17246.0 * e + 4642.0 * f) + e * (7043.0 * e - 3882.0 * f) + 547.0 * (f * f)) / 240.0;
+  const double tau = std::fabs(beta[3] - (beta[0] + beta[2] + 4.0 * beta[1]) / 6.0);   /* eq. (27) */
+  if (indicators) {
+    for (int r = 0; r < 4; ++r) indicators[r] = beta[r];
+    indicators[4] = tau;
+  }
+  double g[4], gsum = 0.0;
+  for (int r = 0; r < 4; ++r) {
+    const double x = 1.0 + tau / (beta[r] + eps);          /* eq. (25), C = 1, q = 6 */
+    const double x2 = x * x;
+    g[r] = x2 * x2 * x2;
+    gsum += g[r];
+  }
+  double dsum = 0.0, del[4], m = std::numeric_limits<double>::infinity();
+  for (int r = 0; r < 4; ++r) {
+    const double chi = g[r] / gsum;                        /* eq. (24) */
+    del[r] = chi < ct ? 0.0 : 1.0;
+    m = std::fmin(m, std::fabs(chi / ct - 1.0));
+    dsum += dw[r] * del[r];
+  }
+  if (margin) *margin = m;
+  double v = 0.0;
+  for (int r = 0; r < 4; ++r) v += dw[r] * del[r] / dsum * q[r];   /* eq. (23), (15) */
+  return v;
+}
+
 /* ---------------------------------------------------------- Roe-averaged eigensystem ---- */
 /* PAPER.md:104-105, steps 2(a)-(b).  Roe average: u_j and H with sqrt(rho) weights, a~ from
  * H~ (Q11).  Eigenvectors for a general unit normal n without tangent vectors
@@ -254,8 +305,14 @@ void interface_flux(const oracle_params *p, const Grid &g, const double *Q, int 
     }
     /* step 2(e): g+ from the left-biased stencil, g- from its mirror image (Q4) */
     double m1, m2;
-    const double hp = reconstruct(p->scheme, gp[0], gp[1], gp[2], gp[3], gp[4], p->eps, p->teno_ct, &m1);
-    const double hm = reconstruct(p->scheme, gm[5], gm[4], gm[3], gm[2], gm[1], p->eps, p->teno_ct, &m2);
+    double hp, hm;
+    if (p->scheme == ORACLE_TENO6) {
+      hp = reconstruct6(gp[0], gp[1], gp[2], gp[3], gp[4], gp[5], p->eps, p->teno_ct, &m1);
+      hm = reconstruct6(gm[5], gm[4], gm[3], gm[2], gm[1], gm[0], p->eps, p->teno_ct, &m2);
+    } else {
+      hp = reconstruct(p->scheme, gp[0], gp[1], gp[2], gp[3], gp[4], p->eps, p->teno_ct, &m1);
+      hm = reconstruct(p->scheme, gm[5], gm[4], gm[3], gm[2], gm[1], p->eps, p->teno_ct, &m2);
+    }
     mmin = std::fmin(mmin, std::fmin(m1, m2));
     /* step 2(f): back to physical space, f^ += (g^+ + g^-) r_k */
     const double gk = hp + hm;
@@ -699,6 +756,15 @@ extern "C" {
 double oracle_reconstruct(int32_t scheme, double a, double b, double c, double d, double e,
                           double eps, double teno_ct, double *margin) {
   return reconstruct(scheme, a, b, c, d, e, eps, teno_ct, margin);
+}
+
+double oracle_reconstruct6(double a, double b, double c, double d, double e, double f,
+                           double eps, double teno_ct, double *margin) {
+  return reconstruct6(a, b, c, d, e, f, eps, teno_ct, margin);
+}
+
+void oracle_teno6_indicators(double a, double b, double c, double d, double e, double f, double *out5) {
+  reconstruct6(a, b, c, d, e, f, 1e-16, 1e-6, nullptr, out5);
 }
 
 void oracle_eigensystem(double gamma, const double *QL, const double *QR, const double *nhat,

@@ -31,7 +31,7 @@
 extern "C" {
 #endif
 
-enum { ORACLE_WENOZ5 = 0, ORACLE_TENO5 = 1 };
+enum { ORACLE_WENOZ5 = 0, ORACLE_TENO5 = 1, ORACLE_TENO6 = 2 };
 enum { ORACLE_VISC_NONE = 0, ORACLE_VISC_CONST = 1, ORACLE_VISC_SUTHERLAND = 2 };
 enum { ORACLE_BC_PERIODIC = 0, ORACLE_BC_EXTRAP0 = 1, ORACLE_BC_DIRICHLET = 2, ORACLE_BC_WALL_ISOTHERMAL = 3 };
 enum { ORACLE_PART_INVISCID = 1, ORACLE_PART_VISCOUS = 2 };
@@ -44,7 +44,7 @@ typedef struct {
   const double *detJ;     /* det(d x / d xi)                                                        */
   const double *E[3][6];  /* E[l][ij] = d2 xi_l / dx_i dx_j, ij in {xx,xy,xz,yy,yz,zz}              */
   double  gamma, Re, Pr, Minf;
-  int32_t scheme;         /* ORACLE_WENOZ5 | ORACLE_TENO5                                           */
+  int32_t scheme;         /* ORACLE_WENOZ5 | ORACLE_TENO5 | ORACLE_TENO6                            */
   double  teno_ct;        /* C_T                                                      */
   double  eps;            /* epsilon of eq. (22), (25)                           */
   int32_t visc;           /* ORACLE_VISC_*                                                          */
@@ -63,6 +63,14 @@ typedef struct {
  * +inf for WENO-Z. */
 double oracle_reconstruct(int32_t scheme, double a, double b, double c, double d, double e,
                           double eps, double teno_ct, double *margin);
+
+/* W6(a,b,c,d,e,f): TENO6 reconstruction at the interface between c and d, upwind side a,b,c
+ * (eq. 23-25 and 27; candidates, ideal weights and beta_3: DESIGN.md Q32). */
+double oracle_reconstruct6(double a, double b, double c, double d, double e, double f,
+                           double eps, double teno_ct, double *margin);
+
+/* beta_0 (R), beta_1 (C), beta_2 (L), beta_3 (4-point) and tau_6 of W6, for the pins. */
+void oracle_teno6_indicators(double a, double b, double c, double d, double e, double f, double *out5);
 
 /* Roe-averaged eigensystem at an interface (step 2a-2b).  QL, QR: the two
  * 5-component conservative states; nhat: unit normal.  Outputs row-major 5x5 L (rows = left

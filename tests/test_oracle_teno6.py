@@ -1,0 +1,121 @@
+"""Pins of the oracle's TENO6 reconstruction (oracle_reconstruct6; eq. 23-25, 27).
+
+The paper prints neither the 4-point candidate, nor the ideal weights, nor beta_3 of the 6th-order
+scheme (refs [20, 21]); Q32 derives them from definitions the paper does give.  Each
+derived piece is pinned here by something other than the oracle's own formula:
+  * candidates and beta_r: symbolic integration of the Jiang-Shu definition [36] on the interpolating
+    polynomials (sympy), compared with oracle_teno6_indicators;
+  * ideal weights: with every stencil kept W6 must be the 6th-order interface value
+    (a - 8b + 37c + 37d - 8e + f)/60, read off by differentiating W6 about a ramp;
+  * order: (W6_{i+1/2} - W6_{i-1/2})/h -> f'(x_i) with error h^6 f^(7)/140 on sin x;
+  * cut-off: a step keeps only stencils that do not cross it; eq. (27) for tau_6;
+  * the residual built on it: conservation and mirror symmetry on a periodic line.
+"""
+import numpy as np
+import pytest
+import sympy as sp
+
+from oracle import oracle as O
+from paper_2007_14933_b200 import workloads as W
+
+
+def _jiang_shu(cells, values):
+    """(interface value at x = +1/2, beta) of the polynomial whose cell averages over the unit cells
+    centred at `cells` are `values`; beta = sum_l int_{-1/2}^{1/2} (d^l p / dx^l)^2 dx."""
+    x = sp.symbols("x")
+    n = len(cells)
+    co = sp.symbols(f"a0:{n}")
+    p = sum(co[k] * x ** k for k in range(n))
+    eqs = [sp.integrate(p, (x, c - sp.Rational(1, 2), c + sp.Rational(1, 2))) - v for c, v in zip(cells, values)]
+    p = p.subs(sp.solve(eqs, co))
+    beta = sum(sp.integrate(sp.diff(p, x, l) ** 2, (x, -sp.Rational(1, 2), sp.Rational(1, 2))) for l in range(1, n))
+    return p.subs(x, sp.Rational(1, 2)), beta
+
+
+def test_indicators_match_the_jiang_shu_definition():
+    rng = np.random.default_rng(6)
+    for _ in range(4):
+        v = [sp.Rational(int(t), 16) for t in rng.integers(-40, 40, size=6)]
+        a, b, c, d, e, f = v
+        exact = [_jiang_shu([0, 1, 2], [c, d, e])[1], _jiang_shu([-1, 0, 1], [b, c, d])[1],
+                 _jiang_shu([-2, -1, 0], [a, b, c])[1], _jiang_shu([0, 1, 2, 3], [c, d, e, f])[1]]
+        tau = abs(exact[3] - (exact[0] + exact[2] + 4 * exact[1]) / 6)               # eq. (27)
+        got = O.teno6_indicators(*[float(t) for t in v])
+        np.testing.assert_allclose(got[:4], [float(t) for t in exact], rtol=1e-13)
+        np.testing.assert_allclose(got[4], float(tau), rtol=1e-11, atol=1e-12)
+
+
+def test_four_point_candidate_is_selected_alone_and_is_the_cubic_value():
+    """Data smooth (a cubic) on {c,d,e,f} only, with a jump in front of c: the 3-point stencils that
+    reach into the jump are cut, and the kept ones (R and the 4-point stencil) reproduce the cubic."""
+    x = sp.symbols("x")
+    poly = 1 + x / 3 - x ** 2 / 7 + x ** 3 / 50
+    avg = [float(sp.integrate(poly, (x, k - sp.Rational(1, 2), k + sp.Rational(1, 2)))) for k in range(4)]
+    val = O.reconstruct6(40.0, -25.0, avg[0], avg[1], avg[2], avg[3])
+    # R = quadratic on {c,d,e}, 4-point = the cubic itself: combined with weights 6/10, 4/10
+    qR = float(_jiang_shu([0, 1, 2], [sp.nsimplify(t) for t in avg[:3]])[0])
+    q4 = float(poly.subs(x, sp.Rational(1, 2)))
+    assert abs(val - (0.6 * qR + 0.4 * q4)) < 1e-13
+    assert abs(float(_jiang_shu([0, 1, 2, 3], [sp.nsimplify(t) for t in avg])[0]) - q4) < 1e-13
+
+
+def test_all_stencils_kept_gives_the_sixth_order_linear_scheme():
+    base = [0.5 * k for k in range(6)]
+    w0 = O.reconstruct6(*base)
+    coef = []
+    for j in range(6):
+        v = list(base)
+        v[j] += 1e-3
+        coef.append((O.reconstruct6(*v) - w0) / 1e-3)
+    np.testing.assert_allclose(coef, np.array([1, -8, 37, 37, -8, 1]) / 60.0, atol=1e-11)
+
+
+@pytest.mark.parametrize("N", [16, 32, 64, 128])
+def test_sixth_order_on_sine(N):
+    h = 2 * np.pi / N
+    x = h * np.arange(N)
+    f = np.sin(x)
+    fh = np.array([O.reconstruct6(*[f[(i + m) % N] for m in range(-2, 4)]) for i in range(N)])    # f^_{i+1/2}
+    err = np.abs((fh - np.roll(fh, 1)) / h - np.cos(x)).max()
+    assert abs(err / (h ** 6 / 140.0) - 1.0) < (0.15 if N == 16 else 0.05), err         # leading term -h^6 f^(7)/140
+
+
+def test_step_and_mirror():
+    assert O.reconstruct6(1, 1, 1, 0, 0, 0) == 1.0            # upwind side smooth: stencils across the jump are cut
+    assert O.reconstruct6(0, 0, 0, 1, 1, 1) == 0.0
+    v, m = O.reconstruct6(0.0, 0.1, 0.3, 0.2, 0.25, 0.4, with_margin=True)
+    assert np.isfinite(v) and m > 0
+
+
+def _line(n=48, scheme=W.TENO6):
+    i, j, k = W.padded_index_grids((n, 1, 1))
+    x = 2 * np.pi * i / n + 0 * j + 0 * k
+    rho = 1.0 + 0.3 * np.sin(x) + 0.1 * np.cos(3 * x)
+    u = 0.4 + 0.2 * np.sin(2 * x + 0.3)
+    p = 1.0 + 0.2 * np.cos(x - 0.5)
+    per = (W.BC_PERIODIC, W.BC_PERIODIC)
+    return W.Case(name="line", n=(n, 1, 1), Q0=np.ascontiguousarray(W.conservative(rho, u, 0.0, 0.0, p, 1.4)), dt=1e-3,
+                  nsteps=1, delta=(2 * np.pi / n, 1.0, 1.0), gamma=1.4, scheme=scheme, bc=(per, (0, 0), (0, 0)))
+
+
+def test_residual_conservation_and_reflection():
+    case = _line()
+    orc = O.Oracle(**case.physics())
+    Q = orc.bc(case.Q0.copy())
+    R = orc.interior(orc.rhs(Q))
+    for c in (0, 1, 4):
+        assert abs(R[c].sum()) <= 1e-12 * np.abs(R[c]).sum()
+    # x -> -x, u -> -u reflects the residual (f- is reconstructed on the mirrored stencil)
+    Qm = orc.interior(case.Q0)[:, :, :, ::-1].copy()
+    Qm[1] *= -1.0
+    case_m = _line()
+    Qpad = case_m.Q0.copy()
+    h = case_m.halo
+    Qpad[:, :, :, h[0]:h[0] + case_m.n[0]] = Qm
+    Rm = orc.interior(orc.rhs(orc.bc(Qpad)))
+    np.testing.assert_allclose(Rm[0][..., ::-1], R[0], rtol=0, atol=1e-12)
+    np.testing.assert_allclose(-Rm[1][..., ::-1], R[1], rtol=0, atol=1e-12)
+    # and TENO6 differs from TENO5 only at truncation level on this smooth line
+    R5 = O.Oracle(**{**case.physics(), "scheme": W.TENO5})
+    R5 = R5.interior(R5.rhs(R5.bc(case.Q0.copy())))
+    assert 1e-9 < np.abs(R5 - R).max() < 1e-2
