@@ -29,7 +29,8 @@ METRIC = "fp64 grid-point RK-stage updates/s at 256^3 TGV"
 UNIT = "updates/s"
 # Algorithmic flop per grid point (restated in DESIGN.md "Roofline"): every add /
 # mul / compare / max / div / sqrt = 1 flop, counted on a CSE'd scalar statement of the method.
-FLOP_SWEEP = {0: 1256 + 15 + 19, 1: 1356 + 15 + 19}      # WENO-Z5, TENO5: interface + difference + primitives
+FLOP_SWEEP = {0: 1256 + 15 + 19, 1: 1356 + 15 + 19,      # WENO-Z5, TENO5: interface + difference + primitives
+              2: 1856 + 15 + 19}                          # TENO6: + ~50 per reconstruction (hand count)
 FLOP_VISCOUS = 300
 FLOP_RK = 20
 
@@ -118,11 +119,11 @@ def ncu_traffic_bytes(kernel):
     return None
 
 
-def cpu_oracle_rate(n, nsteps=1):
+def cpu_oracle_rate(n, nsteps=1, scheme=1):
     """One RK3 step of the n^3 TGV with the oracle as it stands, all host cores."""
     from oracle import oracle as O
     from paper_2007_14933_b200 import workloads as W
-    case = W.tgv(n)
+    case = W.tgv(n, scheme=scheme)
     orc = O.Oracle(**case.physics())
     Q = case.Q0.copy()
     import numpy as np
@@ -185,7 +186,8 @@ def run_ours(args):
     from paper_2007_14933_b200 import workloads as W
 
     n = args.n
-    case = W.tgv(n)
+    scheme = {"wenoz5": W.WENOZ5, "teno5": W.TENO5, "teno6": W.TENO6}[args.scheme]
+    case = W.tgv(n, scheme=scheme)
     sol = osbli.Solver(device=dev, **case.physics())
     hQ = sol.to_padded(case.Q0, pinned_host=True)
     Q = hQ.to(dev)
@@ -291,13 +293,13 @@ def run_ours(args):
     }
 
     cpu_n = 256 if n >= 256 else n          # one RK3 step of the same field: about 10 s on 16 cores at 256^3
-    cpu_rate, cpu_cores, cpu_dt = cpu_oracle_rate(cpu_n)
+    cpu_rate, cpu_cores, cpu_dt = cpu_oracle_rate(cpu_n, scheme=scheme)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"TGV {n}^3 periodic, TENO5 + central-4 viscous, low-storage RK3, dt={case.dt} "
-                               f"(BASELINE.json config {3 if n == 256 else '?'})",
+        "config": {"workload": f"TGV {n}^3 periodic, {args.scheme.upper()} + central-4 viscous, low-storage RK3, dt={case.dt} "
+                               f"(BASELINE.json config {3 if (n == 256 and args.scheme == 'teno5') else ('5' if (n == 512 and args.scheme == 'teno5') else '?')})",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"state {state_bytes / 1e9:.2f} GB per array >> 126 MB L2 (inputs larger than L2)"},
         "clocks": clocks,
@@ -323,6 +325,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=256, help="grid points per side (256 = BASELINE.json config 3)")
+    ap.add_argument("--scheme", default="teno5", choices=["wenoz5", "teno5", "teno6"],
+                    help="reconstruction (teno5 = BASELINE.json config 3; the others are side measurements)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

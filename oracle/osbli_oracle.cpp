@@ -141,7 +141,8 @@ double reconstruct(int scheme, double a, double b, double c, double d, double e,
  *   - d_r: the weights for which sum_r d_r q_r is the 6th-order value (a-8b+37c+37d-8e+f)/60:
  *     d_0 (R) = 6/20, d_1 (C) = 9/20, d_2 (L) = 1/20, d_3 = 4/20;
  *   - beta_3: the Jiang-Shu indicator [36] of that cubic, sum_l dx^(2l-1) int (d^l p/dx^l)^2 dx over
- *     the cell of c (re-derived symbolically in tests/test_oracle_teno6.py).
+ *     the cell of c (re-derived symbolically in tests/test_oracle_teno6.py), evaluated as a sum of
+ *     products of difference combinations like the printed eq. (17)-(19).
  * beta_0 -> R, beta_1 -> C, beta_2 -> L as in eq. (17)-(19). */
 double reconstruct6(double a, double b, double c, double d, double e, double f,
                     double eps, double ct, double *margin, double *indicators = nullptr) {
@@ -155,8 +156,14 @@ double reconstruct6(double a, double b, double c, double d, double e, double f,
   beta[0] = 13.0 / 12.0 * (s0 * s0) + 0.25 * (t0 * t0);   /* eq. (17) */
   beta[1] = 13.0 / 12.0 * (s1 * s1) + 0.25 * (t1 * t1);   /* eq. (18) */
   beta[2] = 13.0 / 12.0 * (s2 * s2) + 0.25 * (t2 * t2);   /* eq. (19) */
-  beta[3] = (c * (2107.0 * c - 9402.0 * d + 7042.0 * e - 1854.0 * f) +
-             d * (11003.0 * d - 17246.0 * e + 4642.0 * f) + e * (7043.0 * e - 3882.0 * f) + 547.0 * (f * f)) / 240.0;
+  /* beta_3 in the form of eq. (17)-(19) (which are a_1^2 + 13/3 a_2^2 of the quadratics): with
+   * a_1, a_2, a_3 the Taylor coefficients of the cubic at the centre of cell c,
+   * beta_3 = a_1^2 + 13/3 a_2^2 + 3129/80 a_3^2 + a_1 a_3 / 2.  Expanded it is the usual
+   * (2107 c^2 - 9402 cd + ... + 547 f^2)/240, which loses ~(c/dc)^2 digits to cancellation. */
+  const double a1 = (-43.0 * c + 69.0 * d - 33.0 * e + 7.0 * f) / 24.0;
+  const double a2 = (2.0 * c - 5.0 * d + 4.0 * e - f) / 2.0;
+  const double a3 = (-c + 3.0 * d - 3.0 * e + f) / 6.0;
+  beta[3] = a1 * a1 + 13.0 / 3.0 * (a2 * a2) + 3129.0 / 80.0 * (a3 * a3) + 0.5 * (a1 * a3);
   const double tau = std::fabs(beta[3] - (beta[0] + beta[2] + 4.0 * beta[1]) / 6.0);   /* eq. (27) */
   if (indicators) {
     for (int r = 0; r < 4; ++r) indicators[r] = beta[r];

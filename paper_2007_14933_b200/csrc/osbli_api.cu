@@ -50,7 +50,7 @@ int validate(const osbli_params *p) {
   Layout L;
   if (int rc = make_layout(p, &L)) return rc;
   if (p->nx == 1) return OSBLI_EUNSUPPORTED;                       // x is the contiguous direction; it must be active
-  if (p->scheme != OSBLI_SCHEME_WENOZ5 && p->scheme != OSBLI_SCHEME_TENO5) return OSBLI_EINVAL;
+  if (p->scheme < OSBLI_SCHEME_WENOZ5 || p->scheme > OSBLI_SCHEME_TENO6) return OSBLI_EINVAL;
   if (p->visc < OSBLI_VISC_NONE || p->visc > OSBLI_VISC_SUTHERLAND) return OSBLI_EINVAL;
   if (!(p->gamma > 1.0)) return OSBLI_EINVAL;
   if (!(p->eps >= 1e-18) || !(p->teno_ct > 0.0)) return OSBLI_EINVAL;
@@ -221,7 +221,8 @@ int osbli_init(const osbli_params *p, void *d_workspace, size_t workspace_bytes,
   P.cq = p->visc != OSBLI_VISC_NONE ? 1.0 / ((p->gamma - 1.0) * p->Minf * p->Minf * p->Pr * p->Re) : 0.0;
   P.scheme = p->scheme; P.visc = p->visc;
   P.ct = p->teno_ct; P.eps = p->eps; P.suth = p->suth_ratio;
-  P.teno_kfast = (std::pow(3.0 * p->teno_ct, -1.0 / 6.0) - 1.0) * (1.0 - 1e-6);
+  const double nstencils = p->scheme == OSBLI_SCHEME_TENO6 ? 4.0 : 3.0;
+  P.teno_kfast = (std::pow(nstencils * p->teno_ct, -1.0 / 6.0) - 1.0) * (1.0 - 1e-6);
   P.dirichlet = p->dirichlet;
   if (p->metrics) {
     for (int k = 0; k < 3; ++k) {

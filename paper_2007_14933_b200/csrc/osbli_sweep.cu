@@ -373,6 +373,8 @@ cudaError_t launch_sweep(const DevParams &P, int dir, const double *Q, double *R
   OSBLI_DISPATCH(1, false)
   OSBLI_DISPATCH(0, true)
   OSBLI_DISPATCH(1, true)
+  OSBLI_DISPATCH(2, false)
+  OSBLI_DISPATCH(2, true)
 #undef OSBLI_DISPATCH
   return cudaErrorInvalidValue;
 }

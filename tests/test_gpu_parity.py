@@ -41,7 +41,7 @@ def run_residual_case(name, case, Q0=None, **over):
         np.testing.assert_allclose(Qg, Qo, rtol=1e-13, atol=1e-14)
     else:
         assert np.array_equal(Qg, Qo), f"{name}: halo fill differs"
-    mi = parity.interior(case, mg) if scheme == W.TENO5 else None
+    mi = parity.interior(case, mg) if scheme in (W.TENO5, W.TENO6) else None
     parity.check_residual(name, case, parity.interior(case, Qo), parity.interior(case, Rg),
                           parity.interior(case, Ro), metrics, margin_i=mi)
     sol.close()
@@ -55,9 +55,10 @@ def test_residual_sod_initial_and_developed():
     Q = orc.run(case.Q0.copy(), case.dt, 150)
     run_residual_case("sod_t0.03", case, Q0=Q)
     run_residual_case("sod_t0.03_teno", case, Q0=Q, scheme=W.TENO5)
+    run_residual_case("sod_t0.03_teno6", case, Q0=Q, scheme=W.TENO6)
 
 
-@pytest.mark.parametrize("scheme", [W.TENO5, W.WENOZ5])
+@pytest.mark.parametrize("scheme", [W.TENO5, W.WENOZ5, W.TENO6])
 @pytest.mark.parametrize("visc", [W.VISC_NONE, W.VISC_CONST])
 def test_residual_tgv32(scheme, visc):
     case = W.tgv(32, scheme=scheme, visc=visc)
@@ -90,6 +91,7 @@ def test_residual_ragged_sizes_span_tiles():
     big.name = "ragged"
     run_residual_case("ragged_teno", big)
     run_residual_case("ragged_wenoz_perturbed", big, Q0=W.perturb(big, seed=9, amp=0.05), scheme=W.WENOZ5)
+    run_residual_case("ragged_teno6_perturbed", big, Q0=W.perturb(big, seed=11, amp=0.05), scheme=W.TENO6)
 
 
 def test_residual_2d_and_nonperiodic_closures():
@@ -115,7 +117,7 @@ def test_residual_curvilinear_euler_wave():
     run_residual_case("wave48_teno", W.euler_wave(48, scheme=W.TENO5))
 
 
-@pytest.mark.parametrize("scheme", [W.WENOZ5, W.TENO5])
+@pytest.mark.parametrize("scheme", [W.WENOZ5, W.TENO5, W.TENO6])
 def test_residual_curvilinear_3d_walls_sutherland(scheme):
     case = W.wavy_box(n=(70, 21, 9), scheme=scheme)
     run_residual_case(f"wavy_box_s{scheme}", case)
@@ -218,6 +220,14 @@ def test_sbli_slab_config4():
     Qg, Qo = run_steps_case(f"sbli_slab_{nsteps}", case, nsteps, 1e-9, parity.l1_rel)
     # the developed state feeds one more residual comparison (shock and boundary layer no longer at rest)
     run_residual_case(f"sbli_slab_after_{nsteps}", case, Q0=Qo)
+
+
+def test_steps_teno6():
+    """SURVEY.md 8(f) NEXT-1: sixth-order TENO through the whole step (fused update, periodic write-through;
+    Sod with extrapolation ends on the 1-D path), same tolerances as the TENO5 configurations."""
+    run_steps_case("tgv32_10_teno6", W.tgv(32, scheme=W.TENO6), 10, 1e-9, parity.q28)
+    run_steps_case("sod_300_teno6", W.sod(scheme=W.TENO6), 300, 1e-9, parity.l1_rel)
+    run_steps_case("wavy_box_5_teno6", W.wavy_box(n=(40, 21, 9), scheme=W.TENO6), 5, 1e-9, parity.l1_rel)
 
 
 def test_advance_host_matches_device_steps():
