@@ -22,6 +22,10 @@ namespace osbli {
 #ifndef OSBLI_YZ_MINB
 #define OSBLI_YZ_MINB 1
 #endif
+__device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+}
 #ifndef OSBLI_X_MINB
 #define OSBLI_X_MINB 1
 #endif
@@ -58,6 +62,7 @@ __global__ void __launch_bounds__(128, CURV ? 1 : OSBLI_YZ_MINB)
 sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
                 int chunk, const RkArgs rk) {
   static_assert(DIR == 1 || DIR == 2, "x has its own kernel");
+  __shared__ double stg[3][5][128];     // per-thread slots: R, dU of node q; Q of node q+4
   const Layout &Ly = P.L;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= Ly.n[0]) return;
@@ -109,30 +114,50 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
     if (m >= 3) rsq[m - 3] = rs;
     if (m == 3) rl = roe_side<CURV>(w[3], rs);   // node s0-1 = left node of the first interface
   }
-  double qn[5], Kn[3];
-  load(s0 + 2, qn, Kn);                          // prefetched raw state of the next node
+  // fused update on uniform grids: the next node's state is staged by cp.async too (measured: helps the
+  // fused z sweep, 0.98 -> 0.95 ms, costs the plain y sweep 0.84 -> 0.85 ms)
+  constexpr bool kAsyncQ = !CURV && RK != 0;
+  auto load_async = [&](int node) {
+    const long long o = line0 + (long long)node * st;
+#pragma unroll
+    for (int c = 0; c < 5; ++c) cp_async8(&stg[2][c][threadIdx.x], Q + c * sv + o);
+  };
+  double qn[5], Kn[3] = {0.0, 0.0, 0.0};
+  if constexpr (kAsyncQ) { load_async(s0 + 2); asm volatile("cp.async.commit_group;" ::: "memory"); }
+  else load(s0 + 2, qn, Kn);                     // prefetched raw state of the next node
 
   for (int q = s0 - 1; q < s1; ++q) {            // interface q+1/2, between nodes q and q+1
 #pragma unroll
     for (int m = 0; m < 5; ++m) w[m] = w[m + 1];
     rsq[0] = rsq[1]; rsq[1] = rsq[2];
+    if constexpr (kAsyncQ) {
+      asm volatile("cp.async.wait_all;" ::: "memory");
+#pragma unroll
+      for (int c = 0; c < 5; ++c) qn[c] = stg[2][c][threadIdx.x];
+    }
     make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], w[5], rsq[2]);
-    if (q + 1 < s1) load(q + 4, qn, Kn);         // node (q+1)+3, used by the next interface
-    // R of node q is read now and consumed after the flux: its latency hides behind ~600 DFMAs.
-    // dU of the fused update is only prefetched into L1 here and loaded after the flux (holding it
-    // in registers as well costs more than the late L1 hit: measured).
-    double rold[5] = {0, 0, 0, 0, 0};
+    if constexpr (!kAsyncQ) {
+      if (q + 1 < s1) load(q + 4, qn, Kn);       // node (q+1)+3, used by the next interface
+    }
+    // R (and dU) of node q travel to per-thread shared-memory slots by cp.async while the flux is
+    // computed: no registers held, no wait until the values are needed
     if (q >= s0) {
       const long long o = line0 + (long long)q * st;
       if constexpr (ACCUM) {
 #pragma unroll
-        for (int c = 0; c < 5; ++c) rold[c] = R[c * sv + o];
+        for (int c = 0; c < 5; ++c) cp_async8(&stg[0][c][threadIdx.x], R + c * sv + o);
       }
       if constexpr (RK == 2) {
 #pragma unroll
-        for (int c = 0; c < 5; ++c) prefetch_l1(rk.Qtmp + c * sv + o);
+        for (int c = 0; c < 5; ++c) cp_async8(&stg[1][c][threadIdx.x], rk.Qtmp + c * sv + o);
       }
     }
+    asm volatile("cp.async.commit_group;" ::: "memory");       // group 1: R, dU of node q (may be empty)
+    if constexpr (kAsyncQ) {
+      if (q + 1 < s1) load_async(q + 4);                       // group 2: node (q+1)+3 for the next interface
+      asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+    double rold[5] = {0, 0, 0, 0, 0};
     const RoeSide rr = roe_side<CURV>(w[3], rsq[0]);
     double f[5];
     if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, rl, rr, rp, f);
@@ -142,11 +167,17 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
       const long long o = line0 + (long long)q * st;
       double sc = inv_d;
       if constexpr (CURV) sc = 1.0 / __ldg(P.detJ + o);
+      if constexpr (kAsyncQ) asm volatile("cp.async.wait_group 1;" ::: "memory");   // group 1 done, group 2 may still fly
+      else asm volatile("cp.async.wait_all;" ::: "memory");
+      if constexpr (ACCUM) {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) rold[c] = stg[0][c][threadIdx.x];
+      }
       if constexpr (RK != 0) {
         double dold[5] = {0, 0, 0, 0, 0};
         if constexpr (RK == 2) {
 #pragma unroll
-          for (int c = 0; c < 5; ++c) dold[c] = rk.Qtmp[c * sv + o];
+          for (int c = 0; c < 5; ++c) dold[c] = stg[1][c][threadIdx.x];
         }
 #pragma unroll
         for (int c = 0; c < 5; ++c) {
