@@ -22,10 +22,6 @@ namespace osbli {
 #ifndef OSBLI_YZ_MINB
 #define OSBLI_YZ_MINB 1
 #endif
-__device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
-}
 #ifndef OSBLI_X_MINB
 #define OSBLI_X_MINB 1
 #endif

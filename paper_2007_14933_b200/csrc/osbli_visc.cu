@@ -260,7 +260,11 @@ constexpr int kVX = 32, kVY = 8, kVH = 2;
 constexpr int kVPX = kVX + 2 * kVH, kVPY = kVY + 2 * kVH;        // 36 x 12 plane tile
 constexpr int kVRing = 4;
 
-struct VSmem { double f[kVRing][4][kVPY][kVPX]; };
+struct VSmem {
+  double f[kVRing][4][kVPY][kVPX];     // ring of u, v, w, T planes (tile + 2-deep x/y halo)
+  double r[4][kVX * kVY];              // per-thread slots: R of the node in flight
+  double raw[5][2][kVX * kVY];         // per-thread slots: raw state of the (up to) two tile points staged next
+};
 
 __global__ void __launch_bounds__(kVX * kVY, 2)
 viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
@@ -288,23 +292,29 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
     // clamp to the halo-extended domain: clamped points are never used by live threads
     pv[s] = pv[s] && (x0 + xx - kVH) < L.n[0] + kVH && (y0 + yy - kVH) < L.n[1] + kVH;
   }
-  auto fetch = [&](int plane, double (&q)[2][5]) {
+  // raw state of this thread's tile points of one plane: global -> per-thread shared-memory slots by
+  // cp.async (no registers in flight), converted to u, v, w, T one step later by the same thread
+  auto fetch = [&](int plane) {
 #pragma unroll
     for (int s = 0; s < 2; ++s)
       if (pv[s]) {
         const long long at = L.at(x0 + pi[s] - kVH, y0 + pj[s] - kVH, plane);
 #pragma unroll
-        for (int c = 0; c < 5; ++c) q[s][c] = __ldg(Q + c * sv + at);
+        for (int c = 0; c < 5; ++c) cp_async8(&S.raw[c][s][tid], Q + c * sv + at);
       }
+    asm volatile("cp.async.commit_group;" ::: "memory");
   };
-  auto stage = [&](int plane, const double (&q)[2][5]) {
+  auto stage = [&](int plane) {
+    asm volatile("cp.async.wait_all;" ::: "memory");
     const int slot = (plane + 8) & (kVRing - 1);
 #pragma unroll
     for (int s = 0; s < 2; ++s)
       if (pv[s]) {
-        const double ir = fast_rcp(q[s][0]);
-        const double u = q[s][1] * ir, v = q[s][2] * ir, w = q[s][3] * ir;
-        const double p = P.gm1 * (q[s][4] - 0.5 * (q[s][1] * u + q[s][2] * v + q[s][3] * w));
+        const double q0 = S.raw[0][s][tid], q1 = S.raw[1][s][tid], q2 = S.raw[2][s][tid], q3 = S.raw[3][s][tid];
+        const double q4 = S.raw[4][s][tid];
+        const double ir = fast_rcp(q0);
+        const double u = q1 * ir, v = q2 * ir, w = q3 * ir;
+        const double p = P.gm1 * (q4 - 0.5 * (q1 * u + q2 * v + q3 * w));
         S.f[slot][0][pj[s]][pi[s]] = u;
         S.f[slot][1][pj[s]][pi[s]] = v;
         S.f[slot][2][pj[s]][pi[s]] = w;
@@ -328,24 +338,26 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
   // (staged one step earlier) enters the register windows and plane k is the centre of the
   // in-plane stencils -- so staging, global loads and the stencil arithmetic of a step are
   // independent of each other and the barrier closes the step.
-  double qn[2][5];
-  fetch(z0 - 2, qn);
-  stage(z0 - 2, qn);
-  fetch(z0 - 1, qn);
+  fetch(z0 - 2);
+  stage(z0 - 2);
+  fetch(z0 - 1);
   __syncthreads();
   const int X = tx + kVH, Y = ty + kVH;
 
   for (int k = z0 - 4; k < z1; ++k) {
     if (k > z0 - 4) __syncthreads();
-    if (k + 3 < z1 + 2) stage(k + 3, qn);
-    if (k + 4 < z1 + 2) fetch(k + 4, qn);
-    double rold[4] = {0, 0, 0, 0};
+    if (k + 3 < z1 + 2) stage(k + 3);
+    // R of node k goes to a per-thread shared-memory slot by cp.async (held in registers it was spilled
+    // right behind the load, a full-latency stall)
     long long at = 0;
     if (k >= z0 && inside) {
       at = L.at(i, j, k);
 #pragma unroll
-      for (int c = 0; c < 4; ++c) rold[c] = R[(c + 1) * sv + at];
+      for (int c = 0; c < 4; ++c) cp_async8(&S.r[c][tid], R + (c + 1) * sv + at);
     }
+    asm volatile("cp.async.commit_group;" ::: "memory");       // group 1: R of node k
+    if (k + 4 < z1 + 2) fetch(k + 4);                          // group 2: raw plane k+4
+    else asm volatile("cp.async.commit_group;" ::: "memory");
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
       uw[m] = uw[m + 1]; vw[m] = vw[m + 1]; ww[m] = ww[m + 1]; Tw[m] = Tw[m + 1];
@@ -415,6 +427,8 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
     const double heat = P.cq * (T_xx + T_yy + T_zz);
     const double r1 = M0 * P.inv_Re, r2 = M1 * P.inv_Re, r3 = M2 * P.inv_Re;
     const double r4 = fma(u, r1, fma(v, r2, w * r3)) + fma(phi, P.inv_Re, heat);
+    asm volatile("cp.async.wait_group 1;" ::: "memory");       // R has landed, the next plane may still fly
+    const double rold[4] = {S.r[0][tid], S.r[1][tid], S.r[2][tid], S.r[3][tid]};
     R[sv + at] = rold[0] + r1;
     R[2 * sv + at] = rold[1] + r2;
     R[3 * sv + at] = rold[2] + r3;
