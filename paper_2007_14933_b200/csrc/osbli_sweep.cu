@@ -250,28 +250,22 @@ sweep_x_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q
   const RecPar rp = make_recpar(P);
   const double inv_d = P.inv_delta[0];
 
-  // The staged rows are a ring of 8 columns (node n in column n & 7), refilled in halves of 4 nodes
-  // by cp.async as soon as a half has been consumed: the copy of nodes [b, b+4) of all 32 rows
-  // (each instruction 8 rows x 32 bytes, whole sectors) flies while the other half is processed
-  // (4 interfaces ~ 7000 cycles), so the march never waits for global memory.
-  const int hr = lane >> 2, hc = lane & 3;
-  const int lr = lane >> 3, lc = lane & 7;                       // store_tile: each instruction moves 4 rows of 64 bytes
-  auto issue_half = [&](int b) {                                 // nodes [b, b+4), b a multiple of 4
+  // cooperative tile load: 32 rows x 8 points, each instruction moves 4 rows of 64 bytes
+  const int lr = lane >> 3, lc = lane & 7;
+  auto load_tile = [&](int a) {                                  // points [a, a+8), a multiple of 8
 #pragma unroll
-    for (int it = 0; it < 4; ++it) {
-      const int rr_ = it * 8 + hr;
-      const long long ro = __shfl_sync(0xffffffffu, row, rr_) + b + hc;
-      const int col = (b + hc) & (kXT - 1);
+    for (int it = 0; it < 8; ++it) {
+      const int rr_ = it * 4 + lr;
+      const long long ro = __shfl_sync(0xffffffffu, row, rr_) + a + lc;
 #pragma unroll
-      for (int c = 0; c < 5; ++c) cp_async8(&S.in[c][rr_][col], Q + c * sv + ro);
+      for (int c = 0; c < 5; ++c) S.in[c][rr_][lc] = __ldg(Q + c * sv + ro);
       if constexpr (CURV) {
-        cp_async8(&S.in[5][rr_][col], P.detJ + ro);
-        cp_async8(&S.in[6][rr_][col], P.D[0][0] + ro);
-        cp_async8(&S.in[7][rr_][col], P.D[0][1] + ro);
-        cp_async8(&S.in[8][rr_][col], P.D[0][2] + ro);
+        S.in[5][rr_][lc] = __ldg(P.detJ + ro);
+        S.in[6][rr_][lc] = __ldg(P.D[0][0] + ro);
+        S.in[7][rr_][lc] = __ldg(P.D[0][1] + ro);
+        S.in[8][rr_][lc] = __ldg(P.D[0][2] + ro);
       }
     }
-    asm volatile("cp.async.commit_group;" ::: "memory");
   };
   auto store_tile = [&](int a) {                                 // flux differences of points [a, a+8) ∩ [s0, s1)
 #pragma unroll
@@ -298,18 +292,18 @@ sweep_x_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q
 #pragma unroll
   for (int m = 0; m < 6; ++m) { w[m].r = 1.0; w[m].m[0] = w[m].m[1] = w[m].m[2] = 0.0; w[m].E = 1.0; w[m].p = 1.0; w[m].th = 0.0; w[m].c = 1.0; }
 
-  {
-    const int b0 = (s0 - 3) - ((s0 - 3) & 3);                    // half holding node s0-3 (floor to a multiple of 4)
-    issue_half(b0);
-    issue_half(b0 + 4);
-  }
+  int a_in = ((s0 - 3) >= 0) ? ((s0 - 3) / kXT) * kXT : -kXT;    // tile holding node s0-3 (s0-3 >= -3)
+  load_tile(a_in);
+  __syncwarp();
 
   for (int node = s0 - 3; node < s1 + 3; ++node) {               // node entering window slot 5
-    if ((node & 3) == 0 || node == s0 - 3) {                     // first node of a half: its copy must have landed
-      asm volatile("cp.async.wait_group 1;" ::: "memory");       // (the younger half may still be in flight)
+    if (node >= a_in + kXT) {
+      __syncwarp();
+      a_in += kXT;
+      load_tile(a_in);
       __syncwarp();
     }
-    const int col = node & (kXT - 1);
+    const int col = node - a_in;
 #pragma unroll
     for (int m = 0; m < 5; ++m) w[m] = w[m + 1];
     rsq[0] = rsq[1]; rsq[1] = rsq[2];
@@ -324,11 +318,6 @@ sweep_x_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q
         Jw[3] = J;
       }
       make_point<0, CURV>(P, r, mx, my, mz, E, kx, ky, kz, w[5], rsq[2]);
-    }
-    if ((node & 3) == 3) {                                       // this half of the ring is consumed: refill it
-      __syncwarp();
-      if (node + 5 < s1 + 3) issue_half(node + 5);               // nodes [node+5, node+9) -> the same four columns
-      else asm volatile("cp.async.commit_group;" ::: "memory");  // (keeps the group count uniform)
     }
     const int q = node - 3;                                      // interface q+1/2 is now computable
     if (q == s0 - 2) rl = roe_side<CURV>(w[3], rsq[0]);         // slot 3 holds node s0-1
