@@ -165,6 +165,22 @@ def run_reference(args):
     return 0
 
 
+def max_over_ranks(ms, device=None):
+    """Device time of the slowest rank (replicas only: no data-path collective)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return ms
+    t = torch.tensor([ms], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_updates_per_s(npoints, steps, world, ms):
+    """Whole-job throughput: every replica advanced npoints x 3 stages x steps in the slowest rank's time."""
+    return world * npoints * 3 * steps / (ms * 1e-3)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -201,13 +217,6 @@ def run_ours(args):
             dist.barrier()
             torch.cuda.synchronize(dev)
 
-    def max_over_ranks(ms):
-        if world == 1:
-            return ms
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
     peak_tflops = sol.measure_fp64_peak() if rank == 0 else 0.0
 
     for _ in range(max(args.warmup, 3)):
@@ -229,7 +238,7 @@ def run_ours(args):
         sol.rk3_step(Q, Qtmp, case.dt)
     e1.record(stream)
     barrier()
-    ms = max_over_ranks(e0.elapsed_time(e1))
+    ms = max_over_ranks(e0.elapsed_time(e1), dev)
     launches = sol.launch_count() - l0
     clocks = sampler.stop() if rank == 0 else None
     assert bool(torch.isfinite(Q).all()), "state blew up"
@@ -253,7 +262,7 @@ def run_ours(args):
         sol.advance_host(hQ, Q, Qtmp, case.dt, 1)
     t1.record(stream)
     barrier()
-    ms_e2e = max_over_ranks(t0.elapsed_time(t1))
+    ms_e2e = max_over_ranks(t0.elapsed_time(t1), dev)
 
     if rank != 0:
         if world > 1:
@@ -261,9 +270,8 @@ def run_ours(args):
         return 0
 
     npts = case.npoints
-    updates = world * npts * 3 * args.steps
-    value = updates / (ms * 1e-3)
-    e2e_value = world * npts * 3 * e2e_steps / (ms_e2e * 1e-3)
+    value = aggregate_updates_per_s(npts, args.steps, world, ms)
+    e2e_value = aggregate_updates_per_s(npts, e2e_steps, world, ms_e2e)
 
     # dominant kernel = the sweep direction with the largest device time
     dom = max(("sweep_x", "sweep_y", "sweep_z"), key=lambda k: prof[k][0])

@@ -1,0 +1,180 @@
+"""P12: an independently written, vectorised NumPy statement of the whole residual on tiny grids.
+
+The other pins fix the oracle's parts (reconstruction, eigenvectors, stencils, boundary fills, RK3);
+this one fixes their assembly -- indices, signs, which point feeds which stencil slot, the order of
+the sweeps -- by writing the algorithm of PAPER.md:100-111 and eq. (2)-(5), (10), (13)-(19), (22)-(29)
+a second time in a different shape: whole-array operations on periodically rolled copies, dense 5x5
+eigenvector matrices applied with einsum, no loops over points.  It shares nothing with
+oracle/osbli_oracle.cpp (triple loops, one interface at a time) beyond the paper.
+
+Uniform grids, periodic boxes in 1-D, 2-D and 3-D, WENO-Z5 / TENO5 / TENO6, mu = 1 viscous terms.
+(Closures, wall and Dirichlet fills, Sutherland and metric terms are pinned on their own: P6, P11,
+P4/P8/P9, P10.)
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2007_14933_b200 import workloads as W
+
+G = 1.4
+
+
+def prim(Q):
+    rho = Q[0]
+    vel = Q[1:4] / rho
+    p = (G - 1.0) * (Q[4] - 0.5 * rho * (vel ** 2).sum(0))
+    return rho, vel, p
+
+
+def weights_and_value(pts, scheme, eps=1e-16, ct=1e-6):
+    """pts: the stencil values [a, b, c, d, e(, f)], upwind side a, b, c; interface between c and d."""
+    a, b, c, d, e = pts[:5]
+    q = [(2 * c + 5 * d - e) / 6, (-b + 5 * c + 2 * d) / 6, (2 * a - 7 * b + 11 * c) / 6]
+    beta = [13 / 12 * (c - 2 * d + e) ** 2 + (3 * c - 4 * d + e) ** 2 / 4,
+            13 / 12 * (b - 2 * c + d) ** 2 + (b - d) ** 2 / 4,
+            13 / 12 * (a - 2 * b + c) ** 2 + (a - 4 * b + 3 * c) ** 2 / 4]
+    dw = [0.3, 0.6, 0.1]
+    tau = np.abs(beta[0] - beta[2])
+    if scheme == W.TENO6:
+        f = pts[5]
+        q.append((3 * c + 13 * d - 5 * e + f) / 12)
+        a1, a2, a3 = (-43 * c + 69 * d - 33 * e + 7 * f) / 24, (2 * c - 5 * d + 4 * e - f) / 2, (-c + 3 * d - 3 * e + f) / 6
+        beta.append(a1 ** 2 + 13 / 3 * a2 ** 2 + 3129 / 80 * a3 ** 2 + a1 * a3 / 2)
+        dw = [0.3, 0.45, 0.05, 0.2]
+        tau = np.abs(beta[3] - (beta[0] + beta[2] + 4 * beta[1]) / 6)
+    if scheme == W.WENOZ5:
+        al = [dw[r] * (1 + (tau / (beta[r] + eps)) ** 2) for r in range(3)]
+    else:
+        gam = [(1 + tau / (beta[r] + eps)) ** 6 for r in range(len(q))]
+        gs = sum(gam)
+        al = [dw[r] * np.where(gam[r] / gs < ct, 0.0, 1.0) for r in range(len(q))]
+    s = sum(al)
+    return sum(al[r] / s * q[r] for r in range(len(q)))
+
+
+def eigenvectors(ut, H, a, n):
+    """Dense L (rows) and R (columns) of SURVEY.md 8(c) O2.3 for unit normal n; arrays [..., 5, 5]."""
+    u, v, w = ut
+    nx, ny, nz = n
+    q2 = u * u + v * v + w * w
+    th = nx * u + ny * v + nz * w
+    b1 = (G - 1) / a ** 2
+    b2 = 0.5 * b1 * q2
+    one, zero = np.ones_like(u), np.zeros_like(u)
+    R = np.stack([
+        np.stack([nx * one, u * nx, v * nx + nz, w * nx - ny, 0.5 * q2 * nx + v * nz - w * ny], -1),
+        np.stack([ny * one, u * ny - nz, v * ny, w * ny + nx, 0.5 * q2 * ny + w * nx - u * nz], -1),
+        np.stack([nz * one, u * nz + ny, v * nz - nx, w * nz, 0.5 * q2 * nz + u * ny - v * nx], -1),
+        np.stack([one, u + a * nx, v + a * ny, w + a * nz, H + a * th], -1),
+        np.stack([one, u - a * nx, v - a * ny, w - a * nz, H - a * th], -1)], -1)          # [..., component, field]
+    L = np.stack([
+        np.stack([nx * (1 - b2) - (v * nz - w * ny), nx * b1 * u, nx * b1 * v + nz, nx * b1 * w - ny, -nx * b1 * one], -1),
+        np.stack([ny * (1 - b2) - (w * nx - u * nz), ny * b1 * u - nz, ny * b1 * v, ny * b1 * w + nx, -ny * b1 * one], -1),
+        np.stack([nz * (1 - b2) - (u * ny - v * nx), nz * b1 * u + ny, nz * b1 * v - nx, nz * b1 * w, -nz * b1 * one], -1),
+        0.5 * np.stack([b2 - th / a, -b1 * u + nx / a, -b1 * v + ny / a, -b1 * w + nz / a, b1 * one], -1),
+        0.5 * np.stack([b2 + th / a, -b1 * u - nx / a, -b1 * v - ny / a, -b1 * w - nz / a, b1 * one], -1)], -2)   # [..., field, component]
+    return L, R, zero
+
+
+def inviscid_sweep(Q, d, delta, scheme):
+    """-(f^_{i+1/2} - f^_{i-1/2})/delta along direction d (0 = x: last axis) on a periodic interior array."""
+    ax = -1 - d
+    n = np.zeros(3)
+    n[d] = 1.0
+    at = lambda A, m: np.roll(A, -m, axis=ax)                      # value at node i + m
+    rho, vel, p = prim(Q)
+    a = np.sqrt(G * p / rho)
+    th = vel[d]
+    F = np.stack([rho * th, Q[1] * th + p * n[0], Q[2] * th + p * n[1], Q[3] * th + p * n[2], (Q[4] + p) * th])
+    lam = [th, th, th, th + a, th - a]
+    # Roe average of nodes i, i+1
+    wl, wr = np.sqrt(rho), np.sqrt(at(rho, 1))
+    ut = (wl * vel + wr * at(vel, 1)) / (wl + wr)
+    Hn = (Q[4] + p) / rho
+    H = (wl * Hn + wr * at(Hn, 1)) / (wl + wr)
+    ar = np.sqrt((G - 1) * (H - 0.5 * (ut ** 2).sum(0)))
+    L, R, _ = eigenvectors(ut, H, ar, n)
+    ms = list(range(-2, 4))
+    V = [np.einsum("...kc,c...->...k", L, at(Q, m)) for m in ms]    # [..., field] at stencil point m
+    Gc = [np.einsum("...kc,c...->...k", L, at(F, m)) for m in ms]
+    alpha = np.stack([np.max(np.stack([np.abs(at(lam[k], m)) for m in ms]), 0) for k in range(5)], -1)
+    gp = [0.5 * (Gc[j] + alpha * V[j]) for j in range(6)]
+    gm = [0.5 * (Gc[j] - alpha * V[j]) for j in range(6)]
+    npts = 6 if scheme == W.TENO6 else 5
+    ghat = weights_and_value(gp[:npts], scheme) + weights_and_value(gm[::-1][:npts], scheme)
+    fhat = np.einsum("...ck,...k->c...", R, ghat)                   # f^_{i+1/2}, component first
+    return -(fhat - np.roll(fhat, 1, axis=ax)) / delta
+
+
+def viscous(Q, delta, Re, Pr, M, active):
+    rho, vel, p = prim(Q)
+    T = G * M * M * p / rho
+
+    def d1(f, k):
+        if not active[k]:
+            return np.zeros_like(f)
+        r = lambda m: np.roll(f, -m, axis=-1 - k)
+        return (r(-2) - 8 * r(-1) + 8 * r(1) - r(2)) / (12 * delta[k])
+
+    def d2(f, k):
+        if not active[k]:
+            return np.zeros_like(f)
+        r = lambda m: np.roll(f, -m, axis=-1 - k)
+        return (-r(-2) + 16 * r(-1) - 30 * f + 16 * r(1) - r(2)) / (12 * delta[k] ** 2)
+
+    dd = lambda f, k, l: d2(f, k) if k == l else d1(d1(f, max(k, l)), min(k, l))     # delta_k(delta_l f), k < l
+    grad = [[d1(vel[i], j) for j in range(3)] for i in range(3)]
+    div = grad[0][0] + grad[1][1] + grad[2][2]
+    Mi = [sum(d2(vel[i], j) for j in range(3)) + sum(dd(vel[k], i, k) for k in range(3)) / 3 for i in range(3)]
+    out = np.zeros_like(Q)
+    for i in range(3):
+        out[1 + i] = Mi[i] / Re
+    phi = sum((grad[i][j] + grad[j][i] - (2 / 3 * div if i == j else 0.0)) * grad[i][j] for i in range(3) for j in range(3)) / Re
+    cq = 1.0 / ((G - 1) * M * M * Pr * Re)
+    out[4] = sum(vel[i] * Mi[i] for i in range(3)) / Re + phi + cq * sum(d2(T, j) for j in range(3))
+    return out
+
+
+def brute_residual(case, scheme, visc):
+    h, n = case.halo, case.n
+    Q = case.Q0[:, h[2]:h[2] + n[2], h[1]:h[1] + n[1], h[0]:h[0] + n[0]].copy()
+    active = [v > 1 for v in n]
+    R = np.zeros_like(Q)
+    for d in range(3):
+        if active[d]:
+            R += inviscid_sweep(Q, d, case.delta[d], scheme)
+    if visc:
+        R += viscous(Q, case.delta, case.Re, case.Pr, case.Minf, active)
+    return R
+
+
+def box(n, seed):
+    rng = np.random.default_rng(seed)
+    i, j, k = W.padded_index_grids(n)
+    x, y, z = 2 * np.pi * i / n[0], 2 * np.pi * j / n[1], 2 * np.pi * k / n[2]
+    ph = rng.uniform(0, 2 * np.pi, 8)
+    rho = 1.0 + 0.3 * np.sin(x + ph[0]) * np.cos(y + ph[1]) + 0.1 * np.cos(z + ph[2])
+    u = 0.5 * np.sin(x + y + ph[3]) + 0.2 * np.cos(z + ph[4])
+    v = (0.4 * np.cos(x - y + ph[5]) + 0.0 * z) if n[1] > 1 else 0.0 * x
+    w = (0.3 * np.sin(z + x + ph[6]) + 0.0 * y) if n[2] > 1 else 0.0 * x
+    p = 1.0 + 0.3 * np.cos(x + ph[7]) * np.sin(y + z)
+    # one steep feature so that the nonlinear weights (and the TENO cut-off) actually do something
+    rho = rho + 0.8 * (np.tanh(4 * np.sin(x)) > 0.5)
+    per = (W.BC_PERIODIC, W.BC_PERIODIC)
+    bc = tuple(per if n[d] > 1 else (0, 0) for d in range(3))
+    return W.Case(name="brute", n=n, Q0=np.ascontiguousarray(W.conservative(rho, u, v, w, p, G)), dt=1e-3, nsteps=1,
+                  delta=tuple(2 * np.pi / v_ for v_ in n), gamma=G, Re=50.0, Pr=0.71, Minf=0.7, bc=bc)
+
+
+@pytest.mark.parametrize("scheme", [W.WENOZ5, W.TENO5, W.TENO6])
+@pytest.mark.parametrize("n", [(8, 6, 5), (12, 10, 1), (16, 1, 1)])
+@pytest.mark.parametrize("visc", [W.VISC_NONE, W.VISC_CONST])
+def test_p12_oracle_equals_vectorised_numpy(scheme, n, visc):
+    case = box(n, seed=sum(n) + scheme)
+    orc = O.Oracle(**{**case.physics(), "scheme": scheme, "visc": visc})
+    Ro = orc.interior(orc.rhs(orc.bc(case.Q0.copy())))
+    Rb = brute_residual(case, scheme, visc != W.VISC_NONE)
+    scale = np.abs(Ro).max(axis=(1, 2, 3), keepdims=True)
+    scale = np.where(scale < 1e-12 * scale.max(), scale.max(), scale)
+    assert (np.abs(Ro - Rb) / scale).max() < 1e-12, (np.abs(Ro - Rb) / scale).max(axis=(1, 2, 3))
