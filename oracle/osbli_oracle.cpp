@@ -97,6 +97,15 @@ double reconstruct(int scheme, double a, double b, double c, double d, double e,
 
   if (margin) *margin = std::numeric_limits<double>::infinity();
 
+  if (scheme == ORACLE_WENOJS5) {
+    /* eq. (20)-(21): alpha_r = d_r / (eps + beta_r)^p, p = 2 (eps = 1e-6 there) */
+    const double aR = dR / ((eps + bR) * (eps + bR));
+    const double aC = dC / ((eps + bC) * (eps + bC));
+    const double aL = dL / ((eps + bL) * (eps + bL));
+    const double sum = aR + aC + aL;
+    return aR / sum * qR + aC / sum * qC + aL / sum * qL;         /* eq. (15), (20) */
+  }
+
   if (scheme == ORACLE_WENOZ5) {
     /* eq. (22): alpha_r = d_r (1 + (tau/(beta_r+eps))^2), omega_r = alpha_r/sum */
     const double rR = tau / (bR + eps), rC = tau / (bC + eps), rL = tau / (bL + eps);

@@ -31,7 +31,7 @@
 extern "C" {
 #endif
 
-enum { ORACLE_WENOZ5 = 0, ORACLE_TENO5 = 1, ORACLE_TENO6 = 2 };
+enum { ORACLE_WENOZ5 = 0, ORACLE_TENO5 = 1, ORACLE_TENO6 = 2, ORACLE_WENOJS5 = 3 };
 enum { ORACLE_VISC_NONE = 0, ORACLE_VISC_CONST = 1, ORACLE_VISC_SUTHERLAND = 2 };
 enum { ORACLE_BC_PERIODIC = 0, ORACLE_BC_EXTRAP0 = 1, ORACLE_BC_DIRICHLET = 2, ORACLE_BC_WALL_ISOTHERMAL = 3 };
 enum { ORACLE_PART_INVISCID = 1, ORACLE_PART_VISCOUS = 2 };
@@ -44,7 +44,7 @@ typedef struct {
   const double *detJ;     /* det(d x / d xi)                                                        */
   const double *E[3][6];  /* E[l][ij] = d2 xi_l / dx_i dx_j, ij in {xx,xy,xz,yy,yz,zz}              */
   double  gamma, Re, Pr, Minf;
-  int32_t scheme;         /* ORACLE_WENOZ5 | ORACLE_TENO5 | ORACLE_TENO6                            */
+  int32_t scheme;         /* ORACLE_WENOZ5 | ORACLE_TENO5 | ORACLE_TENO6 | ORACLE_WENOJS5           */
   double  teno_ct;        /* C_T                                                      */
   double  eps;            /* epsilon of eq. (22), (25)                           */
   int32_t visc;           /* ORACLE_VISC_*                                                          */

@@ -7,7 +7,7 @@ a second time in a different shape: whole-array operations on periodically rolle
 eigenvector matrices applied with einsum, no loops over points.  It shares nothing with
 oracle/osbli_oracle.cpp (triple loops, one interface at a time) beyond the paper.
 
-Uniform grids, periodic boxes in 1-D, 2-D and 3-D, WENO-Z5 / TENO5 / TENO6, mu = 1 viscous terms.
+Uniform grids, periodic boxes in 1-D, 2-D and 3-D, WENO-Z5 / TENO5 / TENO6 / WENO-JS5, mu = 1 viscous terms.
 (Closures, wall and Dirichlet fills, Sutherland and metric terms are pinned on their own: P6, P11,
 P4/P8/P9, P10.)
 """
@@ -43,7 +43,9 @@ def weights_and_value(pts, scheme, eps=1e-16, ct=1e-6):
         beta.append(a1 ** 2 + 13 / 3 * a2 ** 2 + 3129 / 80 * a3 ** 2 + a1 * a3 / 2)
         dw = [0.3, 0.45, 0.05, 0.2]
         tau = np.abs(beta[3] - (beta[0] + beta[2] + 4 * beta[1]) / 6)
-    if scheme == W.WENOZ5:
+    if scheme == W.WENOJS5:
+        al = [dw[r] / (1e-6 + beta[r]) ** 2 for r in range(3)]       # eq. (21), eps = 1e-6
+    elif scheme == W.WENOZ5:
         al = [dw[r] * (1 + (tau / (beta[r] + eps)) ** 2) for r in range(3)]
     else:
         gam = [(1 + tau / (beta[r] + eps)) ** 6 for r in range(len(q))]
@@ -167,12 +169,12 @@ def box(n, seed):
                   delta=tuple(2 * np.pi / v_ for v_ in n), gamma=G, Re=50.0, Pr=0.71, Minf=0.7, bc=bc)
 
 
-@pytest.mark.parametrize("scheme", [W.WENOZ5, W.TENO5, W.TENO6])
+@pytest.mark.parametrize("scheme", [W.WENOZ5, W.TENO5, W.TENO6, W.WENOJS5])
 @pytest.mark.parametrize("n", [(8, 6, 5), (12, 10, 1), (16, 1, 1)])
 @pytest.mark.parametrize("visc", [W.VISC_NONE, W.VISC_CONST])
 def test_p12_oracle_equals_vectorised_numpy(scheme, n, visc):
     case = box(n, seed=sum(n) + scheme)
-    orc = O.Oracle(**{**case.physics(), "scheme": scheme, "visc": visc})
+    orc = O.Oracle(**{**case.physics(), "scheme": scheme, "visc": visc, "eps": 1e-6 if scheme == W.WENOJS5 else 1e-16})
     Ro = orc.interior(orc.rhs(orc.bc(case.Q0.copy())))
     Rb = brute_residual(case, scheme, visc != W.VISC_NONE)
     scale = np.abs(Ro).max(axis=(1, 2, 3), keepdims=True)
