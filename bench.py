@@ -30,7 +30,8 @@ UNIT = "updates/s"
 # Algorithmic flop per grid point (restated in DESIGN.md "Roofline"): every add /
 # mul / compare / max / div / sqrt = 1 flop, counted on a CSE'd scalar statement of the method.
 FLOP_SWEEP = {0: 1256 + 15 + 19, 1: 1356 + 15 + 19,      # WENO-Z5, TENO5: interface + difference + primitives
-              2: 1856 + 15 + 19}                          # TENO6: + ~50 per reconstruction (hand count)
+              2: 1856 + 15 + 19,                          # TENO6: + ~50 per reconstruction (hand count)
+              3: 1206 + 15 + 19}                          # WENO-JS5: WENO-Z5 minus tau and the (1 + (.)^2) factors
 FLOP_VISCOUS = 300
 FLOP_RK = 20
 
@@ -124,6 +125,8 @@ def cpu_oracle_rate(n, nsteps=1, scheme=1):
     from oracle import oracle as O
     from paper_2007_14933_b200 import workloads as W
     case = W.tgv(n, scheme=scheme)
+    if scheme == W.WENOJS5:
+        case.eps = 1e-6
     orc = O.Oracle(**case.physics())
     Q = case.Q0.copy()
     import numpy as np
@@ -202,8 +205,10 @@ def run_ours(args):
     from paper_2007_14933_b200 import workloads as W
 
     n = args.n
-    scheme = {"wenoz5": W.WENOZ5, "teno5": W.TENO5, "teno6": W.TENO6}[args.scheme]
+    scheme = {"wenoz5": W.WENOZ5, "teno5": W.TENO5, "teno6": W.TENO6, "wenojs5": W.WENOJS5}[args.scheme]
     case = W.tgv(n, scheme=scheme)
+    if scheme == W.WENOJS5:
+        case.eps = 1e-6                                   # eq. (21)
     sol = osbli.Solver(device=dev, **case.physics())
     hQ = sol.to_padded(case.Q0, pinned_host=True)
     Q = hQ.to(dev)
@@ -333,7 +338,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=256, help="grid points per side (256 = BASELINE.json config 3)")
-    ap.add_argument("--scheme", default="teno5", choices=["wenoz5", "teno5", "teno6"],
+    ap.add_argument("--scheme", default="teno5", choices=["wenoz5", "teno5", "teno6", "wenojs5"],
                     help="reconstruction (teno5 = BASELINE.json config 3; the others are side measurements)")
     args = ap.parse_args()
     if args.impl == "reference":

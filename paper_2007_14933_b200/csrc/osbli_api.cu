@@ -50,7 +50,7 @@ int validate(const osbli_params *p) {
   Layout L;
   if (int rc = make_layout(p, &L)) return rc;
   if (p->nx == 1) return OSBLI_EUNSUPPORTED;                       // x is the contiguous direction; it must be active
-  if (p->scheme < OSBLI_SCHEME_WENOZ5 || p->scheme > OSBLI_SCHEME_TENO6) return OSBLI_EINVAL;
+  if (p->scheme < OSBLI_SCHEME_WENOZ5 || p->scheme > OSBLI_SCHEME_WENOJS5) return OSBLI_EINVAL;
   if (p->visc < OSBLI_VISC_NONE || p->visc > OSBLI_VISC_SUTHERLAND) return OSBLI_EINVAL;
   if (!(p->gamma > 1.0)) return OSBLI_EINVAL;
   if (!(p->eps >= 1e-18) || !(p->teno_ct > 0.0)) return OSBLI_EINVAL;

@@ -9,6 +9,9 @@
 // adding  d_j tau_ij,  d_j(u_i tau_ij) - d_j q_j  to R.
 #include "osbli_kernels.h"
 
+#include <cuda.h>          // CUtensorMap (types only; the encoder is fetched through the runtime)
+#include <cstring>
+
 namespace osbli {
 
 // eq. (7): p = (gamma-1)(rhoE - rho u.u/2), T = gamma M^2 p / rho;
@@ -260,17 +263,54 @@ constexpr int kVX = 32, kVY = 8, kVH = 2;
 constexpr int kVPX = kVX + 2 * kVH, kVPY = kVY + 2 * kVH;        // 36 x 12 plane tile
 constexpr int kVRing = 4;
 
-struct VSmem {
+// Raw planes reach shared memory either by TMA (one cp.async.bulk.tensor per plane: the 36 x 12 tile of all
+// five variables is one box of a 4-D tensor map over the state, issued by one thread, completion on an
+// mbarrier, rows past the array are zero-filled by the hardware) or, where no tensor map could be encoded,
+// by per-thread 8-byte cp.async.
+template <bool TMA> struct VSmemT;
+template <> struct VSmemT<false> {
   double f[kVRing][4][kVPY][kVPX];     // ring of u, v, w, T planes (tile + 2-deep x/y halo)
   double r[4][kVX * kVY];              // per-thread slots: R of the node in flight
   double raw[5][2][kVX * kVY];         // per-thread slots: raw state of the (up to) two tile points staged next
 };
+template <> struct VSmemT<true> {
+  double tile[2][5][kVPY][kVPX];       // TMA destinations (128-byte aligned: first member), double buffered
+  double f[kVRing][4][kVPY][kVPX];
+  double r[4][kVX * kVY];
+  unsigned long long mbar[2];          // one mbarrier per TMA buffer
+};
+constexpr unsigned kVTileBytes = 5 * kVPY * kVPX * sizeof(double);
 
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// bounded spin: a transaction count that never completes traps instead of hanging the device
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+  const unsigned a = smem_u32(bar);
+  for (unsigned spin = 0; spin < (1u << 28); ++spin) {
+    unsigned ok;
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    if (ok) return;
+  }
+  __trap();
+}
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, int c3,
+                                            unsigned long long *bar) {
+  asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+               ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+
+template <bool TMA>
 __global__ void __launch_bounds__(kVX * kVY, 2)
 viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
-                   int chunk) {
-  extern __shared__ __align__(16) unsigned char vs_raw[];
-  VSmem &S = *reinterpret_cast<VSmem *>(vs_raw);
+                   int chunk, const __grid_constant__ CUtensorMap tmap) {
+  extern __shared__ __align__(128) unsigned char vs_raw[];
+  VSmemT<TMA> &S = *reinterpret_cast<VSmemT<TMA> *>(vs_raw);
   const Layout &L = P.L;
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * kVX + tx;
   const int x0 = blockIdx.x * kVX, y0 = blockIdx.y * kVY;
@@ -292,26 +332,48 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
     // clamp to the halo-extended domain: clamped points are never used by live threads
     pv[s] = pv[s] && (x0 + xx - kVH) < L.n[0] + kVH && (y0 + yy - kVH) < L.n[1] + kVH;
   }
-  // raw state of this thread's tile points of one plane: global -> per-thread shared-memory slots by
-  // cp.async (no registers in flight), converted to u, v, w, T one step later by the same thread
+  // plane number jj = plane - (z0 - 2) of this block goes through TMA buffer jj & 1; its mbarrier has then
+  // completed (jj >> 1) phases before, which fixes the parity to wait for
   auto fetch = [&](int plane) {
-#pragma unroll
-    for (int s = 0; s < 2; ++s)
-      if (pv[s]) {
-        const long long at = L.at(x0 + pi[s] - kVH, y0 + pj[s] - kVH, plane);
-#pragma unroll
-        for (int c = 0; c < 5; ++c) cp_async8(&S.raw[c][s][tid], Q + c * sv + at);
+    if constexpr (TMA) {
+      if (tid == 0) {
+        const int b = (plane - (z0 - 2)) & 1;
+        mbar_expect_tx(&S.mbar[b], kVTileBytes);
+        tma_load_4d(&S.tile[b][0][0][0], &tmap, (int)L.xoff + x0 - kVH, L.h[1] + y0 - kVH, L.h[2] + plane, 0, &S.mbar[b]);
       }
-    asm volatile("cp.async.commit_group;" ::: "memory");
+    } else {
+      // raw state of this thread's tile points: global -> per-thread shared-memory slots by cp.async (no
+      // registers in flight), converted to u, v, w, T one step later by the same thread
+#pragma unroll
+      for (int s = 0; s < 2; ++s)
+        if (pv[s]) {
+          const long long at = L.at(x0 + pi[s] - kVH, y0 + pj[s] - kVH, plane);
+#pragma unroll
+          for (int c = 0; c < 5; ++c) cp_async8(&S.raw[c][s][tid], Q + c * sv + at);
+        }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");       // (empty with TMA: keeps the group count of the R copies)
   };
   auto stage = [&](int plane) {
-    asm volatile("cp.async.wait_all;" ::: "memory");
     const int slot = (plane + 8) & (kVRing - 1);
+    int b = 0;
+    if constexpr (TMA) {
+      const int jj = plane - (z0 - 2);
+      b = jj & 1;
+      mbar_wait(&S.mbar[b], (unsigned)(jj >> 1) & 1u);
+    } else {
+      asm volatile("cp.async.wait_all;" ::: "memory");
+    }
 #pragma unroll
     for (int s = 0; s < 2; ++s)
       if (pv[s]) {
-        const double q0 = S.raw[0][s][tid], q1 = S.raw[1][s][tid], q2 = S.raw[2][s][tid], q3 = S.raw[3][s][tid];
-        const double q4 = S.raw[4][s][tid];
+        double q0, q1, q2, q3, q4;
+        if constexpr (TMA) {
+          q0 = S.tile[b][0][pj[s]][pi[s]]; q1 = S.tile[b][1][pj[s]][pi[s]]; q2 = S.tile[b][2][pj[s]][pi[s]];
+          q3 = S.tile[b][3][pj[s]][pi[s]]; q4 = S.tile[b][4][pj[s]][pi[s]];
+        } else {
+          q0 = S.raw[0][s][tid]; q1 = S.raw[1][s][tid]; q2 = S.raw[2][s][tid]; q3 = S.raw[3][s][tid]; q4 = S.raw[4][s][tid];
+        }
         const double ir = fast_rcp(q0);
         const double u = q1 * ir, v = q2 * ir, w = q3 * ir;
         const double p = P.gm1 * (q4 - 0.5 * (q1 * u + q2 * v + q3 * w));
@@ -321,6 +383,14 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
         S.f[slot][3][pj[s]][pi[s]] = P.gM2 * p * ir;
       }
   };
+  if constexpr (TMA) {
+    if (tid == 0) {
+      mbar_init(&S.mbar[0], 1);
+      mbar_init(&S.mbar[1], 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+  }
 
   const double cx = P.inv12d[0], cy = P.inv12d[1], cz = P.inv12d[2];
   const double cxx = P.inv12d2[0], cyy = P.inv12d2[1], czz = P.inv12d2[2];
@@ -443,17 +513,56 @@ bool viscous_fast_path(const DevParams &P) {
   return true;
 }
 
+// 4-D tensor map over a state: (x incl. row padding, y incl. halo, z incl. halo, variable), box = one plane
+// tile of all five variables.  The encoder lives in the driver library; it is fetched through the runtime
+// so that libosbli links against nothing but cudart.
+static bool encode_state_map(const Layout &L, const double *Q, CUtensorMap *map) {
+  typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static encode_fn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void *ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<encode_fn>(ptr);
+  }
+  if (!fn) return false;
+  const cuuint64_t dims[4] = {(cuuint64_t)L.sy, (cuuint64_t)(L.n[1] + 2 * L.h[1]), (cuuint64_t)(L.n[2] + 2 * L.h[2]), 5};
+  const cuuint64_t strides[3] = {(cuuint64_t)L.sy * 8, (cuuint64_t)L.sz * 8, (cuuint64_t)L.sv * 8};
+  const cuuint32_t box[4] = {kVPX, kVPY, 1, 5};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double *>(Q), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 cudaError_t launch_viscous_fast(const DevParams &P, const double *Q, double *R, cudaStream_t st) {
   const Layout &L = P.L;
   const int chunk = L.n[2] > OSBLI_VCHUNK ? OSBLI_VCHUNK : L.n[2];
   dim3 grid((L.n[0] + kVX - 1) / kVX, (L.n[1] + kVY - 1) / kVY, (L.n[2] + chunk - 1) / chunk);
   static bool attr_done = false;
   if (!attr_done) {
-    cudaError_t e = cudaFuncSetAttribute(viscous_tgv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(VSmem));
+    cudaError_t e = cudaFuncSetAttribute(viscous_tgv_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(VSmemT<true>));
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(viscous_tgv_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               (int)sizeof(VSmemT<false>));
     if (e != cudaSuccess) return e;
     attr_done = true;
   }
-  viscous_tgv_kernel<<<grid, dim3(kVX, kVY), sizeof(VSmem), st>>>(P, Q, R, chunk);
+  CUtensorMap map;
+#ifndef OSBLI_VISC_NO_TMA
+  if (encode_state_map(L, Q, &map)) {
+    viscous_tgv_kernel<true><<<grid, dim3(kVX, kVY), sizeof(VSmemT<true>), st>>>(P, Q, R, chunk, map);
+    return cudaGetLastError();
+  }
+#endif
+  memset(&map, 0, sizeof(map));
+  viscous_tgv_kernel<false><<<grid, dim3(kVX, kVY), sizeof(VSmemT<false>), st>>>(P, Q, R, chunk, map);
   return cudaGetLastError();
 }
 
