@@ -10,7 +10,6 @@
 #include "osbli_kernels.h"
 
 #include <cuda.h>          // CUtensorMap (types only; the encoder is fetched through the runtime)
-#include <cstring>
 
 namespace osbli {
 
@@ -254,7 +253,8 @@ cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *pr
 // column in registers: u, v, w, T for the z-derivatives, and d_x u, d_y v, d_x w, d_y w so that the
 // x-z / y-z mixed derivatives are z-differences of its own registers.  Only the x-y mixed
 // derivatives and the in-plane stencils read shared memory (84 LDS.64 per node).  One barrier per
-// plane.  R is read at the top of a step and written at its end.
+// plane.  The raw planes arrive by TMA two steps ahead of their use, R of the node by cp.async into a
+// per-thread slot: nothing waits in registers.
 // =============================================================================================
 #ifndef OSBLI_VCHUNK
 #define OSBLI_VCHUNK 32
@@ -263,20 +263,13 @@ constexpr int kVX = 32, kVY = 8, kVH = 2;
 constexpr int kVPX = kVX + 2 * kVH, kVPY = kVY + 2 * kVH;        // 36 x 12 plane tile
 constexpr int kVRing = 4;
 
-// Raw planes reach shared memory either by TMA (one cp.async.bulk.tensor per plane: the 36 x 12 tile of all
-// five variables is one box of a 4-D tensor map over the state, issued by one thread, completion on an
-// mbarrier, rows past the array are zero-filled by the hardware) or, where no tensor map could be encoded,
-// by per-thread 8-byte cp.async.
-template <bool TMA> struct VSmemT;
-template <> struct VSmemT<false> {
-  double f[kVRing][4][kVPY][kVPX];     // ring of u, v, w, T planes (tile + 2-deep x/y halo)
-  double r[4][kVX * kVY];              // per-thread slots: R of the node in flight
-  double raw[5][2][kVX * kVY];         // per-thread slots: raw state of the (up to) two tile points staged next
-};
-template <> struct VSmemT<true> {
+// Raw planes reach shared memory by TMA: the 36 x 12 tile of all five variables of one plane is one box of a
+// 4-D tensor map over the state, loaded by one cp.async.bulk.tensor issued by one thread, completion on an
+// mbarrier; rows and columns past the array are zero-filled by the hardware (ragged tiles need no guards).
+struct VSmem {
   double tile[2][5][kVPY][kVPX];       // TMA destinations (128-byte aligned: first member), double buffered
-  double f[kVRing][4][kVPY][kVPX];
-  double r[4][kVX * kVY];
+  double f[kVRing][4][kVPY][kVPX];     // ring of u, v, w, T planes (tile + 2-deep x/y halo)
+  double r[4][kVX * kVY];              // per-thread slots: R of the node in flight (cp.async)
   unsigned long long mbar[2];          // one mbarrier per TMA buffer
 };
 constexpr unsigned kVTileBytes = 5 * kVPY * kVPX * sizeof(double);
@@ -305,12 +298,11 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, i
                ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
 }
 
-template <bool TMA>
 __global__ void __launch_bounds__(kVX * kVY, 2)
 viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
                    int chunk, const __grid_constant__ CUtensorMap tmap) {
   extern __shared__ __align__(128) unsigned char vs_raw[];
-  VSmemT<TMA> &S = *reinterpret_cast<VSmemT<TMA> *>(vs_raw);
+  VSmem &S = *reinterpret_cast<VSmem *>(vs_raw);
   const Layout &L = P.L;
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * kVX + tx;
   const int x0 = blockIdx.x * kVX, y0 = blockIdx.y * kVY;
@@ -335,45 +327,21 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
   // plane number jj = plane - (z0 - 2) of this block goes through TMA buffer jj & 1; its mbarrier has then
   // completed (jj >> 1) phases before, which fixes the parity to wait for
   auto fetch = [&](int plane) {
-    if constexpr (TMA) {
-      if (tid == 0) {
-        const int b = (plane - (z0 - 2)) & 1;
-        mbar_expect_tx(&S.mbar[b], kVTileBytes);
-        tma_load_4d(&S.tile[b][0][0][0], &tmap, (int)L.xoff + x0 - kVH, L.h[1] + y0 - kVH, L.h[2] + plane, 0, &S.mbar[b]);
-      }
-    } else {
-      // raw state of this thread's tile points: global -> per-thread shared-memory slots by cp.async (no
-      // registers in flight), converted to u, v, w, T one step later by the same thread
-#pragma unroll
-      for (int s = 0; s < 2; ++s)
-        if (pv[s]) {
-          const long long at = L.at(x0 + pi[s] - kVH, y0 + pj[s] - kVH, plane);
-#pragma unroll
-          for (int c = 0; c < 5; ++c) cp_async8(&S.raw[c][s][tid], Q + c * sv + at);
-        }
+    if (tid == 0) {
+      const int b = (plane - (z0 - 2)) & 1;
+      mbar_expect_tx(&S.mbar[b], kVTileBytes);
+      tma_load_4d(&S.tile[b][0][0][0], &tmap, (int)L.xoff + x0 - kVH, L.h[1] + y0 - kVH, L.h[2] + plane, 0, &S.mbar[b]);
     }
-    asm volatile("cp.async.commit_group;" ::: "memory");       // (empty with TMA: keeps the group count of the R copies)
   };
   auto stage = [&](int plane) {
     const int slot = (plane + 8) & (kVRing - 1);
-    int b = 0;
-    if constexpr (TMA) {
-      const int jj = plane - (z0 - 2);
-      b = jj & 1;
-      mbar_wait(&S.mbar[b], (unsigned)(jj >> 1) & 1u);
-    } else {
-      asm volatile("cp.async.wait_all;" ::: "memory");
-    }
+    const int jj = plane - (z0 - 2), b = jj & 1;
+    mbar_wait(&S.mbar[b], (unsigned)(jj >> 1) & 1u);
 #pragma unroll
     for (int s = 0; s < 2; ++s)
       if (pv[s]) {
-        double q0, q1, q2, q3, q4;
-        if constexpr (TMA) {
-          q0 = S.tile[b][0][pj[s]][pi[s]]; q1 = S.tile[b][1][pj[s]][pi[s]]; q2 = S.tile[b][2][pj[s]][pi[s]];
-          q3 = S.tile[b][3][pj[s]][pi[s]]; q4 = S.tile[b][4][pj[s]][pi[s]];
-        } else {
-          q0 = S.raw[0][s][tid]; q1 = S.raw[1][s][tid]; q2 = S.raw[2][s][tid]; q3 = S.raw[3][s][tid]; q4 = S.raw[4][s][tid];
-        }
+        const double q0 = S.tile[b][0][pj[s]][pi[s]], q1 = S.tile[b][1][pj[s]][pi[s]], q2 = S.tile[b][2][pj[s]][pi[s]];
+        const double q3 = S.tile[b][3][pj[s]][pi[s]], q4 = S.tile[b][4][pj[s]][pi[s]];
         const double ir = fast_rcp(q0);
         const double u = q1 * ir, v = q2 * ir, w = q3 * ir;
         const double p = P.gm1 * (q4 - 0.5 * (q1 * u + q2 * v + q3 * w));
@@ -383,14 +351,12 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
         S.f[slot][3][pj[s]][pi[s]] = P.gM2 * p * ir;
       }
   };
-  if constexpr (TMA) {
-    if (tid == 0) {
-      mbar_init(&S.mbar[0], 1);
-      mbar_init(&S.mbar[1], 1);
-      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
+  if (tid == 0) {
+    mbar_init(&S.mbar[0], 1);
+    mbar_init(&S.mbar[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  __syncthreads();
 
   const double cx = P.inv12d[0], cy = P.inv12d[1], cz = P.inv12d[2];
   const double cxx = P.inv12d2[0], cyy = P.inv12d2[1], czz = P.inv12d2[2];
@@ -425,9 +391,8 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
 #pragma unroll
       for (int c = 0; c < 4; ++c) cp_async8(&S.r[c][tid], R + (c + 1) * sv + at);
     }
-    asm volatile("cp.async.commit_group;" ::: "memory");       // group 1: R of node k
-    if (k + 4 < z1 + 2) fetch(k + 4);                          // group 2: raw plane k+4
-    else asm volatile("cp.async.commit_group;" ::: "memory");
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    if (k + 4 < z1 + 2) fetch(k + 4);                          // raw plane k+4 into the buffer plane k+2 has left
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
       uw[m] = uw[m + 1]; vw[m] = vw[m + 1]; ww[m] = ww[m + 1]; Tw[m] = Tw[m + 1];
@@ -497,7 +462,7 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
     const double heat = P.cq * (T_xx + T_yy + T_zz);
     const double r1 = M0 * P.inv_Re, r2 = M1 * P.inv_Re, r3 = M2 * P.inv_Re;
     const double r4 = fma(u, r1, fma(v, r2, w * r3)) + fma(phi, P.inv_Re, heat);
-    asm volatile("cp.async.wait_group 1;" ::: "memory");       // R has landed, the next plane may still fly
+    asm volatile("cp.async.wait_all;" ::: "memory");           // R has landed
     const double rold[4] = {S.r[0][tid], S.r[1][tid], S.r[2][tid], S.r[3][tid]};
     R[sv + at] = rold[0] + r1;
     R[2 * sv + at] = rold[1] + r2;
@@ -546,23 +511,13 @@ cudaError_t launch_viscous_fast(const DevParams &P, const double *Q, double *R, 
   dim3 grid((L.n[0] + kVX - 1) / kVX, (L.n[1] + kVY - 1) / kVY, (L.n[2] + chunk - 1) / chunk);
   static bool attr_done = false;
   if (!attr_done) {
-    cudaError_t e = cudaFuncSetAttribute(viscous_tgv_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)sizeof(VSmemT<true>));
-    if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(viscous_tgv_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               (int)sizeof(VSmemT<false>));
+    cudaError_t e = cudaFuncSetAttribute(viscous_tgv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(VSmem));
     if (e != cudaSuccess) return e;
     attr_done = true;
   }
   CUtensorMap map;
-#ifndef OSBLI_VISC_NO_TMA
-  if (encode_state_map(L, Q, &map)) {
-    viscous_tgv_kernel<true><<<grid, dim3(kVX, kVY), sizeof(VSmemT<true>), st>>>(P, Q, R, chunk, map);
-    return cudaGetLastError();
-  }
-#endif
-  memset(&map, 0, sizeof(map));
-  viscous_tgv_kernel<false><<<grid, dim3(kVX, kVY), sizeof(VSmemT<false>), st>>>(P, Q, R, chunk, map);
+  if (!encode_state_map(L, Q, &map)) return cudaErrorNotSupported;
+  viscous_tgv_kernel<<<grid, dim3(kVX, kVY), sizeof(VSmem), st>>>(P, Q, R, chunk, map);
   return cudaGetLastError();
 }
 
