@@ -44,6 +44,7 @@ class _Params(C.Structure):
         ("wall_T", (C.c_double * 2) * 3),
         ("dirichlet", _dp),
         ("nthreads", C.c_int32),
+        ("force", C.c_double * 3),
     ]
 
 
@@ -186,7 +187,7 @@ class Oracle:
     def __init__(self, *, n, delta=(1.0, 1.0, 1.0), metrics=None, gamma=1.4, Re=1.0, Pr=1.0, Minf=1.0,
                  scheme=WENOZ5, teno_ct=1e-6, eps=1e-16, visc=VISC_NONE, suth_ratio=110.4 / 288.0,
                  bc=((0, 0), (0, 0), (0, 0)), wall_T=((0, 0), (0, 0), (0, 0)), dirichlet=None,
-                 nthreads=None):
+                 nthreads=None, force=(0.0, 0.0, 0.0)):
         self.n = tuple(int(v) for v in n)
         self.h = tuple(3 if v > 1 else 0 for v in self.n)
         self.N = tuple(v + 2 * h for v, h in zip(self.n, self.h))
@@ -226,6 +227,7 @@ class Oracle:
             self._keep.append(a)
             p.dirichlet = _ptr(a)
         p.nthreads = self.nthreads
+        p.force[:] = [float(v) for v in force]
         self.p = p
 
     def _field(self, a):

@@ -676,8 +676,20 @@ void bc_direction(const oracle_params *p, const Grid &g, double *Q, int d) {
           for (int m = 0; m <= 3; ++m)
             for (int c = 0; c < 5; ++c)
               Q[c * g.total + wall - (long)m * inw] = p->dirichlet[c * g.total + wall - (long)m * inw];
-        } else if (type == ORACLE_BC_WALL_ISOTHERMAL) {
-          const double Tw = p->wall_T[d][side];
+        } else if (type == ORACLE_BC_WALL_ISOTHERMAL || type == ORACLE_BC_WALL_ADIABATIC) {
+          double Tw = p->wall_T[d][side];
+          if (type == ORACLE_BC_WALL_ADIABATIC) {
+            /* "a one-sided 4th order approximation of dT/dy = 0 is rearranged using the
+             * interior points to calculate the unknown wall temperature": eq. (30) set to zero,
+             * -25 T_w + 48 T_1 - 36 T_2 + 16 T_3 - 3 T_4 = 0. */
+            double T[5];
+            for (int m = 1; m <= 4; ++m) {
+              double qm[5];
+              load_state(g, Q, wall + (long)m * inw, qm);
+              T[m] = prim_of(p, qm).T;
+            }
+            Tw = (48.0 * T[1] - 36.0 * T[2] + 16.0 * T[3] - 3.0 * T[4]) / 25.0;
+          }
           /* eq. (40)-(41): no-slip on the boundary plane, wall energy from T_w; rho_w floats */
           const double rw = Q[wall];
           Q[1 * g.total + wall] = 0.0;
@@ -760,6 +772,23 @@ void rhs_full(const oracle_params *p, const Grid &g, const double *Q, double *R,
           double r[5] = {0, 0, 0, 0, 0};
           viscous_at(ps, NodeIdx{{i, j, k}}, at, r);
           for (int c = 1; c < 5; ++c) R[c * g.total + at] += r[c];
+        }
+  }
+
+  /* constant body force (Q34): momentum += f, energy += u . f */
+  if ((parts & ORACLE_PART_VISCOUS) && (p->force[0] != 0.0 || p->force[1] != 0.0 || p->force[2] != 0.0)) {
+    for (int k = 0; k < g.n[2]; ++k)
+      for (int j = 0; j < g.n[1]; ++j)
+        for (int i = 0; i < g.n[0]; ++i) {
+          const long at = g.idx(i, j, k);
+          double q[5];
+          load_state(g, Q, at, q);
+          double work = 0.0;
+          for (int a = 0; a < 3; ++a) {
+            R[(1 + a) * g.total + at] += p->force[a];
+            work += q[1 + a] / q[0] * p->force[a];
+          }
+          R[4 * g.total + at] += work;
         }
   }
 }
@@ -846,6 +875,14 @@ int32_t oracle_rhs_points(const oracle_params *p, const double *Q, int32_t parts
       double rv[5] = {0, 0, 0, 0, 0};
       viscous_at(ps, NodeIdx{{i, j, k}}, at, rv);
       for (int c = 1; c < 5; ++c) r[c] += rv[c];
+    }
+    if (parts & ORACLE_PART_VISCOUS) {
+      double q[5];
+      load_state(g, Q, at, q);
+      for (int a = 0; a < 3; ++a) {
+        r[1 + a] += p->force[a];
+        r[4] += q[1 + a] / q[0] * p->force[a];
+      }
     }
     for (int c = 0; c < 5; ++c) out[5 * t + c] = r[c];
   }

@@ -33,7 +33,8 @@ extern "C" {
 
 enum { ORACLE_WENOZ5 = 0, ORACLE_TENO5 = 1, ORACLE_TENO6 = 2, ORACLE_WENOJS5 = 3 };
 enum { ORACLE_VISC_NONE = 0, ORACLE_VISC_CONST = 1, ORACLE_VISC_SUTHERLAND = 2 };
-enum { ORACLE_BC_PERIODIC = 0, ORACLE_BC_EXTRAP0 = 1, ORACLE_BC_DIRICHLET = 2, ORACLE_BC_WALL_ISOTHERMAL = 3 };
+enum { ORACLE_BC_PERIODIC = 0, ORACLE_BC_EXTRAP0 = 1, ORACLE_BC_DIRICHLET = 2, ORACLE_BC_WALL_ISOTHERMAL = 3,
+       ORACLE_BC_WALL_ADIABATIC = 4 };
 enum { ORACLE_PART_INVISCID = 1, ORACLE_PART_VISCOUS = 2 };
 
 typedef struct {
@@ -53,6 +54,8 @@ typedef struct {
   double  wall_T[3][2];   /* T_w of eq. (41)                                                        */
   const double *dirichlet;/* full state (oracle layout) holding frozen boundary values, or NULL     */
   int32_t nthreads;       /* OpenMP threads for the outer line loops (>= 1)                         */
+  double  force[3];       /* constant body force per unit volume (channel case):  */
+                          /* R_{rho u_i} += f_i, R_{rho E} += u_i f_i (Q34)               */
 } oracle_params;
 
 /* ---- building blocks, exposed so that the pins can reach them one by one ---------------- */

@@ -22,7 +22,7 @@ import numpy as np
 
 WENOZ5, TENO5, TENO6, WENOJS5 = 0, 1, 2, 3
 VISC_NONE, VISC_CONST, VISC_SUTHERLAND = 0, 1, 2
-BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL = 0, 1, 2, 3
+BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL, BC_WALL_ADIABATIC = 0, 1, 2, 3, 4
 
 
 @dataclass
@@ -46,6 +46,7 @@ class Case:
     bc: tuple = ((0, 0), (0, 0), (0, 0))
     wall_T: tuple = ((0.0, 0.0), (0.0, 0.0), (0.0, 0.0))
     dirichlet: Optional[np.ndarray] = None     # [5, NZ, NY, NX] frozen boundary state
+    force: tuple = (0.0, 0.0, 0.0)             # constant body force per unit volume
     extra: dict = field(default_factory=dict)  # analytic solutions etc. for the pins
 
     @property
@@ -64,7 +65,8 @@ class Case:
         """Keyword arguments shared by both back-ends' constructors (metrics excluded)."""
         return dict(n=self.n, delta=self.delta, gamma=self.gamma, Re=self.Re, Pr=self.Pr, Minf=self.Minf,
                     scheme=self.scheme, teno_ct=self.teno_ct, eps=self.eps, visc=self.visc,
-                    suth_ratio=self.suth_ratio, bc=self.bc, wall_T=self.wall_T, dirichlet=self.dirichlet)
+                    suth_ratio=self.suth_ratio, bc=self.bc, wall_T=self.wall_T, dirichlet=self.dirichlet,
+                    force=self.force)
 
 
 # ------------------------------------------------------------------------------ helpers ----
@@ -310,6 +312,36 @@ def sbli_slab(n=(500, 250, 8), seed=2007014933, noise=1e-4, dt=1e-3, nsteps=500,
     return Case(name="sbli_slab", n=n, Q0=Q0, dt=dt, nsteps=nsteps, delta=(1.0, 1.0, 1.0), coords=coords, gamma=gamma,
                 Re=Re, Pr=Pr, Minf=M, scheme=scheme, visc=VISC_SUTHERLAND, suth_ratio=S, bc=bc, wall_T=wt,
                 dirichlet=dirichlet, extra={"bl": bl, "x0": x0, "shock": sh})
+
+
+# ------------------------------------------------- laminar channel ----
+def channel(n=(32, 64, 1), Re=90.0, Pr=0.72, M=0.01, scheme=TENO6, dt=1e-4, nsteps=10, noise=0.0, seed=3):
+    """Laminar compressible channel of PAPER.md:535-546: isothermal wall (T = 1) at y = -1, adiabatic wall at
+    y = +1, constant viscosity, periodic in x, driven by a unit body force; initial state = the analytic
+    steady solution eq. (52)-(53) (plus optional seeded noise so that parity inputs are not a fixed point)."""
+    n = tuple(int(v) for v in n)
+    gamma = 1.4
+    i, j, k = padded_index_grids(n)
+    y = -1.0 + 2.0 * j / (n[1] - 1.0) + 0.0 * i + 0.0 * k
+    yc = np.clip(y, -1.0, 1.0)
+    u = Re * (1.0 - yc ** 2) / 2.0                                                   # eq. (52)
+    T = 1.0 - Re ** 2 * M ** 2 * Pr * (gamma - 1.0) * (yc ** 4 - 4.0 * yc - 5.0) / 12.0   # eq. (53)
+    p = 1.0 / (gamma * M * M)
+    rho = 1.0 / T
+    if noise:
+        ii, jj, kk = np.meshgrid(np.arange(-halo_of(n)[0], n[0] + halo_of(n)[0]), np.arange(-halo_of(n)[1], n[1] + halo_of(n)[1]),
+                                 np.arange(-halo_of(n)[2], n[2] + halo_of(n)[2]), indexing="ij")
+        lin = ((ii + 8) + 4096 * ((jj + 8) + 4096 * (kk + 8))).astype(np.uint64)
+        rho = rho * (1.0 + noise * splitmix64_unit(seed, lin).transpose(2, 1, 0))
+        u = u * (1.0 + noise * splitmix64_unit(seed + 1, lin).transpose(2, 1, 0))
+    Q0 = edge_pad_interior(np.ascontiguousarray(conservative(rho, u, 0.0 * u, 0.0 * u, p + 0.0 * u, gamma)), n)
+    per = (BC_PERIODIC, BC_PERIODIC)
+    bc = (per, (BC_WALL_ISOTHERMAL, BC_WALL_ADIABATIC), per if n[2] > 1 else (0, 0))
+    Taw = 1.0 + 8.0 * Re ** 2 * M ** 2 * Pr * (gamma - 1.0) / 12.0
+    return Case(name="channel", n=n, Q0=Q0, dt=dt, nsteps=nsteps,
+                delta=(2.0 * np.pi / n[0], 2.0 / (n[1] - 1.0), (2.0 * np.pi / n[2]) if n[2] > 1 else 1.0), gamma=gamma,
+                Re=Re, Pr=Pr, Minf=M, scheme=scheme, visc=VISC_CONST, bc=bc, wall_T=((0.0, 0.0), (1.0, 0.0), (0.0, 0.0)),
+                force=(1.0, 0.0, 0.0), extra={"T_aw": Taw, "u": u, "T": T})
 
 
 # --------------------------------------------------- small curvilinear box (parity cases) ----
