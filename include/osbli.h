@@ -49,7 +49,7 @@ enum { OSBLI_SCHEME_WENOZ5 = 0, OSBLI_SCHEME_TENO5 = 1, OSBLI_SCHEME_TENO6 = 2,
 enum { OSBLI_VISC_NONE = 0 /* Euler */, OSBLI_VISC_CONST = 1 /* mu = 1 */,
        OSBLI_VISC_SUTHERLAND = 2 /* PAPER.md:59-63, 317-318 */ };
 enum { OSBLI_BC_PERIODIC = 0, OSBLI_BC_EXTRAP0 = 1, OSBLI_BC_DIRICHLET = 2,
-       OSBLI_BC_WALL_ISOTHERMAL = 3 };
+       OSBLI_BC_WALL_ISOTHERMAL = 3, OSBLI_BC_WALL_ADIABATIC = 4 };
 
 /* Curvilinear metric fields, DEVICE pointers, each one scalar field in the
  * padded layout with halos filled.  Unit computational spacing in every direction. */
@@ -80,6 +80,8 @@ typedef struct {
   double  wall_T[3][2];    /* T_w of eq. (41) where bc == OSBLI_BC_WALL_ISOTHERMAL               */
   const double *dirichlet; /* DEVICE pointer to a full state (padded layout) holding the frozen
                               boundary values, required iff some bc == OSBLI_BC_DIRICHLET        */
+  double  force[3];        /* constant body force per unit volume (laminar channel):
+                              dQ/dt gains f_i in the momentum and u_i f_i in the energy equation  */
 } osbli_params;
 
 typedef struct {
@@ -107,7 +109,9 @@ int osbli_init(const osbli_params *p, void *d_workspace, size_t workspace_bytes,
  * place: x, then y over the x-extended range, then z over the x,y-extended range, so edges and
  * corners are defined.  PERIODIC: wrap.  EXTRAP0: zero-order extrapolation of the boundary
  * node.  DIRICHLET: boundary plane + halos copied from params.dirichlet
- * (PAPER.md:493, 586).  WALL_ISOTHERMAL: eq. (40)-(46). */
+ * (PAPER.md:493, 586).  WALL_ISOTHERMAL: eq. (40)-(46).  WALL_ADIABATIC: the same
+ * with T_w = (48 T_1 - 36 T_2 + 16 T_3 - 3 T_4)/25 from the interior nodes of the wall-normal line
+ * (one-sided 4th-order dT/dn = 0). */
 int osbli_bc(osbli_handle h, double *d_Q, void *cuda_stream);
 
 /* d_R <- dQ/dt on interior nodes (halo / pad entries of R untouched):

@@ -60,7 +60,8 @@ int validate(const osbli_params *p) {
     const int n = d == 0 ? p->nx : (d == 1 ? p->ny : p->nz);
     for (int s = 0; s < 2; ++s) {
       const int b = p->bc[d][s];
-      if (b < OSBLI_BC_PERIODIC || b > OSBLI_BC_WALL_ISOTHERMAL) return OSBLI_EINVAL;
+      if (b < OSBLI_BC_PERIODIC || b > OSBLI_BC_WALL_ADIABATIC) return OSBLI_EINVAL;
+      if (n > 1 && b == OSBLI_BC_WALL_ADIABATIC && !(p->Minf > 0.0)) return OSBLI_EINVAL;
       if (n > 1 && b == OSBLI_BC_DIRICHLET) need_dirichlet = true;
       if (n > 1 && b == OSBLI_BC_WALL_ISOTHERMAL && !(p->wall_T[d][s] > 0.0)) return OSBLI_EINVAL;
       if (n > 1 && b == OSBLI_BC_WALL_ISOTHERMAL && !(p->Minf > 0.0)) return OSBLI_EINVAL;
@@ -125,12 +126,14 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
     if (d == last && last > 0) {                                    // viscous terms go in front of the last sweep
       if (fast_visc) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous_fast(P, Q, R, st));
       else if (P.visc != OSBLI_VISC_NONE) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, accumulate, st));
+      if (P.has_force) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_force(P, Q, R, st));
     }
     OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep(P, d, Q, R, accumulate, d == last ? rk : nullptr, st));
     accumulate = 1;
   }
   if (last == 0 && P.visc != OSBLI_VISC_NONE)                       // 1-D: the x sweep, then the viscous terms
     OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, accumulate, st));
+  if (last == 0 && P.has_force) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_force(P, Q, R, st));
   return OSBLI_OK;
 }
 
@@ -224,6 +227,8 @@ int osbli_init(const osbli_params *p, void *d_workspace, size_t workspace_bytes,
   const double nstencils = p->scheme == OSBLI_SCHEME_TENO6 ? 4.0 : 3.0;
   P.teno_kfast = (std::pow(nstencils * p->teno_ct, -1.0 / 6.0) - 1.0) * (1.0 - 1e-6);
   P.dirichlet = p->dirichlet;
+  for (int a = 0; a < 3; ++a) P.force[a] = p->force[a];
+  P.has_force = (p->force[0] != 0.0 || p->force[1] != 0.0 || p->force[2] != 0.0) ? 1 : 0;
   if (p->metrics) {
     for (int k = 0; k < 3; ++k) {
       for (int j = 0; j < 3; ++j) P.D[k][j] = p->metrics->D[k][j];

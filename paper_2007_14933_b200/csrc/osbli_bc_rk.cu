@@ -45,8 +45,16 @@ bc_kernel(const __grid_constant__ DevParams P, double *__restrict__ Q) {
     } else if (type == 2) {            // Dirichlet: boundary plane and halos from the frozen state
       for (int m = 0; m <= 3; ++m)
         for (int c = 0; c < 5; ++c) Q[c * sv + wall - m * inw] = __ldg(P.dirichlet + c * sv + wall - m * inw);
-    } else {                           // isothermal no-slip wall, eq. (40)-(46)
-      const double Tw = P.wall_T[DIR][side];
+    } else {                           // no-slip wall, eq. (40)-(46): isothermal (3) or adiabatic (4)
+      auto temperature = [&](long long a) {
+        const double r = Q[a], mx = Q[sv + a], my = Q[2 * sv + a], mz = Q[3 * sv + a], E = Q[4 * sv + a];
+        const double u = mx / r, v = my / r, w = mz / r;
+        return P.gM2 * (P.gm1 * (E - 0.5 * r * (u * u + v * v + w * w))) / r;
+      };
+      double Tw = P.wall_T[DIR][side];
+      if (type == 4)                   // one-sided 4th-order dT/dn = 0 solved for T_w
+        Tw = (48.0 * temperature(wall + inw) - 36.0 * temperature(wall + 2 * inw) + 16.0 * temperature(wall + 3 * inw) -
+              3.0 * temperature(wall + 4 * inw)) / 25.0;
       const double rw = Q[wall];                             // rho_w floats (continuity)
       Q[sv + wall] = 0.0; Q[2 * sv + wall] = 0.0; Q[3 * sv + wall] = 0.0;   // eq. (40)
       const double Ew = rw * Tw / (P.gM2 * P.gm1);           // eq. (41)
@@ -74,6 +82,29 @@ bc_kernel(const __grid_constant__ DevParams P, double *__restrict__ Q) {
       }
     }
   }
+}
+
+// Constant body force per unit volume (the laminar channel of PAPER.md:535-546; Q34).
+__global__ void __launch_bounds__(128)
+force_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R) {
+  const Layout &L = P.L;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= L.n[0]) return;
+  const long long at = L.at(i, blockIdx.y, blockIdx.z), sv = L.sv;
+  const double ir = 1.0 / Q[at];
+  double work = 0.0;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    R[(1 + a) * sv + at] += P.force[a];
+    work += Q[(1 + a) * sv + at] * ir * P.force[a];
+  }
+  R[4 * sv + at] += work;
+}
+
+cudaError_t launch_force(const DevParams &P, const double *Q, double *R, cudaStream_t st) {
+  dim3 grid((P.L.n[0] + 127) / 128, P.L.n[1], P.L.n[2]);
+  force_kernel<<<grid, 128, 0, st>>>(P, Q, R);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_bc(const DevParams &P, int dir, double *Q, cudaStream_t st) {

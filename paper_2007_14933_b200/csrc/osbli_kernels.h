@@ -24,6 +24,9 @@ cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *pr
 bool viscous_fast_path(const DevParams &P);
 cudaError_t launch_viscous_fast(const DevParams &P, const double *Q, double *R, cudaStream_t st);
 
+// constant body force (osbli_bc_rk.cu): R_{rho u_i} += f_i, R_{rho E} += u_i f_i on interior nodes
+cudaError_t launch_force(const DevParams &P, const double *Q, double *R, cudaStream_t st);
+
 // halo fill along one direction (osbli_bc_rk.cu); returns the number of launches through *nl
 cudaError_t launch_bc(const DevParams &P, int dir, double *Q, cudaStream_t st);
 

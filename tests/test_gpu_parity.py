@@ -36,7 +36,7 @@ def run_residual_case(name, case, Q0=None, **over):
     Ro, mg = orc.rhs(Qo, margin=True)
     Qg, Rg = gpu_residual(sol, Q0)
     # halo fill: copy-type boundaries are bit-exact; the wall formulas agree to rounding
-    has_wall = any(b == W.BC_WALL_ISOTHERMAL for d in range(3) for b in case.bc[d] if case.n[d] > 1)
+    has_wall = any(b in (W.BC_WALL_ISOTHERMAL, W.BC_WALL_ADIABATIC) for d in range(3) for b in case.bc[d] if case.n[d] > 1)
     if has_wall:
         np.testing.assert_allclose(Qg, Qo, rtol=1e-13, atol=1e-14)
     else:
@@ -240,6 +240,17 @@ def test_wenojs5_scheme():
     run_residual_case("wavy_box_wenojs", W.wavy_box(n=(24, 20, 8), scheme=W.WENOJS5), eps=1e-6)
     run_steps_case("tgv32_10_wenojs", case, 10, 1e-9, parity.q28, eps=1e-6)
     run_steps_case("sod_300_wenojs", W.sod(scheme=W.WENOJS5), 300, 1e-9, parity.l1_rel, eps=1e-6)
+
+
+def test_channel_adiabatic_wall_and_body_force():
+    """the laminar channel of PAPER.md:535-546 (isothermal wall below, adiabatic wall
+    above, unit body force, mu = 1), analytic profile plus seeded noise: boundary fill, residual and steps."""
+    case = W.channel(n=(32, 64, 1), noise=1e-3)
+    run_residual_case("channel_teno6", case)
+    run_residual_case("channel_wenoz", case, scheme=W.WENOZ5)
+    run_residual_case("channel3d_teno5", W.channel(n=(24, 33, 6), noise=1e-3, scheme=W.TENO5))
+    run_steps_case("channel_20", case, 20, 1e-9, parity.q28)
+    run_steps_case("channel3d_5", W.channel(n=(24, 33, 6), noise=1e-3, scheme=W.TENO5), 5, 1e-9, parity.q28)
 
 
 def test_advance_host_matches_device_steps():
