@@ -98,6 +98,10 @@ def lib():
         L.oracle_rk3_step.argtypes = [C.POINTER(_Params), _dp, _dp, _dp, C.c_double]
         L.oracle_rk3_update.restype = None
         L.oracle_rk3_update.argtypes = [C.c_int32, C.c_double, C.c_int64, _dp, _dp, _dp]
+        L.oracle_rk4_step.restype = C.c_int32
+        L.oracle_rk4_step.argtypes = [C.POINTER(_Params), _dp, _dp, _dp, C.c_double]
+        L.oracle_rk4_update.restype = None
+        L.oracle_rk4_update.argtypes = [C.c_int32, C.c_double, C.c_int64, _dp, _dp, _dp]
         _lib = L
     return _lib
 
@@ -147,6 +151,11 @@ def d2(f, i, periodic, delta, pad=0):
     n = f.size - 2 * pad
     base = C.cast(C.addressof(_ptr(f).contents) + 8 * pad, _dp)
     return lib().oracle_d2(base, n, i, int(periodic), delta)
+
+
+def rk4_update(s, dt, U, dU, R):
+    """One sub-stage (s = 0..4) of the five-stage 4th-order scheme on flat arrays, in place."""
+    lib().oracle_rk4_update(int(s), float(dt), U.size, _ptr(U), _ptr(dU), _ptr(R))
 
 
 def rk3_update(s, dt, U, dU, R):
@@ -283,10 +292,15 @@ class Oracle:
         assert rc == 0
         return Q
 
-    def run(self, Q, dt, nsteps):
-        """Advance Q in place by nsteps RK3 steps."""
+    def rk4_step(self, Q, dU, R, dt):
+        rc = lib().oracle_rk4_step(C.byref(self.p), _ptr(Q), _ptr(dU), _ptr(R), float(dt))
+        assert rc == 0
+        return Q
+
+    def run(self, Q, dt, nsteps, rk4=False):
+        """Advance Q in place by nsteps RK3 (or five-stage RK4) steps."""
         dU = np.zeros(self.shape)
         R = np.zeros(self.shape)
         for _ in range(nsteps):
-            self.rk3_step(Q, dU, R, dt)
+            (self.rk4_step if rk4 else self.rk3_step)(Q, dU, R, dt)
         return Q

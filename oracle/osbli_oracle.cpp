@@ -910,6 +910,40 @@ void oracle_rk3_update(int32_t s, double dt, int64_t count, double *U, double *d
   }
 }
 
+/* The 4th-order member of the same low-storage family eq. (36)-(38): "The 3rd and 4th order schemes have
+ * three and five sub-stages per iteration respectively. The coefficients A_i and B_i are taken from [23]"
+ * (PAPER.md:242): the five-stage 2N-storage scheme of Carpenter & Kennedy (Q35). */
+void oracle_rk4_update(int32_t s, double dt, int64_t count, double *U, double *dU, const double *R) {
+  const double A[5] = {0.0, -567301805773.0 / 1357537059087.0, -2404267990393.0 / 2016746695238.0,
+                       -3550918686646.0 / 2091501179385.0, -1275806237668.0 / 842570457699.0};
+  const double B[5] = {1432997174477.0 / 9575080441755.0, 5161836677717.0 / 13612068292357.0,
+                       1720146321549.0 / 2090206949498.0, 3134564353537.0 / 4481467310338.0,
+                       2277821191437.0 / 14882151754819.0};
+  for (int64_t o = 0; o < count; ++o) {
+    const double du = (s == 0 ? 0.0 : A[s] * dU[o]) + dt * R[o];               /* eq. (36) */
+    dU[o] = du;
+    U[o] = U[o] + B[s] * du;                                                    /* eq. (37) */
+  }
+}
+
+int32_t oracle_rk4_step(const oracle_params *p, double *Q, double *dU, double *R, double dt) {
+  if (validate(p)) return 1;
+  const Grid g = make_grid(p);
+  for (int s = 0; s < 5; ++s) {
+    for (int d = 0; d < 3; ++d) bc_direction(p, g, Q, d);
+    rhs_full(p, g, Q, R, ORACLE_PART_INVISCID | ORACLE_PART_VISCOUS, nullptr);
+#pragma omp parallel for num_threads(p->nthreads) schedule(static)
+    for (int k = 0; k < g.n[2]; ++k)
+      for (int j = 0; j < g.n[1]; ++j)
+        for (int c = 0; c < 5; ++c) {
+          const long o = c * g.total + g.idx(0, j, k);
+          oracle_rk4_update(s, dt, g.n[0], Q + o, dU + o, R + o);
+        }
+  }
+  for (int d = 0; d < 3; ++d) bc_direction(p, g, Q, d);
+  return 0;
+}
+
 int32_t oracle_rk3_step(const oracle_params *p, double *Q, double *dU, double *R, double dt) {
   if (validate(p)) return 1;
   const Grid g = make_grid(p);

@@ -127,6 +127,10 @@ void oracle_rk3_update(int32_t s, double dt, int64_t count, double *U, double *d
  * dU = A_s dU + dt R; Q += B_s dU }; bc(Q).  dU and R are caller-provided scratch states. */
 int32_t oracle_rk3_step(const oracle_params *p, double *Q, double *dU, double *R, double dt);
 
+/* Five-stage 4th-order member of the same family (Q35). */
+void oracle_rk4_update(int32_t s, double dt, int64_t count, double *U, double *dU, const double *R);
+int32_t oracle_rk4_step(const oracle_params *p, double *Q, double *dU, double *R, double dt);
+
 #ifdef __cplusplus
 }
 #endif
