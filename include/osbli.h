@@ -9,6 +9,7 @@
  *                     characteristic WENO-Z5 / TENO5 + LLF         117-194 (eq. 14-26), 85-98 (eq. 11-13),
  *                     + 4th-order central viscous / heat flux      45-57 (eq. 1-5), 198-228 (eq. 28-35)
  *   - osbli_rk3_step  3-stage low-storage Runge-Kutta step         PAPER.md:232-242 (eq. 36-38)
+ *   - osbli_rk4_step  5-stage 4th-order member of the same family
  *   - osbli_advance_host  same, from/to HOST memory (copies inside)
  *
  * Conventions
@@ -129,6 +130,10 @@ int osbli_rhs(osbli_handle h, const double *d_Q, double *d_R, void *cuda_stream)
  * d_Q through two workspace states; the result is in d_Q with its halos filled.  The viscous
  * terms are added in front of the last sweep.  1-D problems update d_Q in place. */
 int osbli_rk3_step(osbli_handle h, double *d_Q, double *d_Qtmp, double dt, void *cuda_stream);
+
+/* The same with the five-stage 4th-order member of the family eq. (36)-(38) ("The 3rd and
+ * 4th order schemes have three and five sub-stages per iteration"): Q -> Q2 -> Q3 -> Q2 -> Q3 -> Q. */
+int osbli_rk4_step(osbli_handle h, double *d_Q, double *d_Qtmp, double dt, void *cuda_stream);
 
 /* End-to-end convenience with HOST buffers: copies h_Q (host, padded layout, total_doubles
  * doubles) to d_Q, runs nsteps RK3 steps of size dt, copies the state back into h_Q and

@@ -137,28 +137,29 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
   return OSBLI_OK;
 }
 
-// One low-storage RK3 step, eq. (36)-(38).  With two or more active directions the update is fused
-// into the last sweep of every stage, which cannot update in place, so the state moves
-// Q -> Q2 -> Q3 -> Q through two workspace states; 1-D problems use the separate in-place update
-// kernel.  The result is in Q either way.
-int do_step(osbli_ctx *h, double *Q, double *Qtmp, double dt, cudaStream_t st) {
+// One low-storage Runge-Kutta step, eq. (36)-(38), nstages = 3 (RK3) or 5 (4th order).  With two or more
+// active directions the update is fused into the last sweep of every stage, which cannot update in place,
+// so the state moves Q -> Q2 -> Q3 (-> Q2 -> Q3) -> Q through two workspace states; 1-D problems use the
+// separate in-place update kernel.  The result is in Q either way.
+int do_step(osbli_ctx *h, int nstages, double *Q, double *Qtmp, double dt, cudaStream_t st) {
   const bool fuse = h->P.L.n[1] > 1 || h->P.L.n[2] > 1;
   bool wrap = fuse;                  // every active direction periodic: the fused update fills the halos itself
   for (int d = 0; d < 3; ++d)
     if (h->P.L.n[d] > 1 && !h->P.periodic[d]) wrap = false;
-  double *const chain[4] = {Q, h->Q2, h->Q3, Q};
-  for (int s = 0; s < 3; ++s) {
+  for (int s = 0; s < nstages; ++s) {
     if (fuse) {
+      double *src = s == 0 ? Q : ((s & 1) ? h->Q2 : h->Q3);
+      double *dst = s == nstages - 1 ? Q : ((s & 1) ? h->Q3 : h->Q2);
       if (s == 0 || !wrap)
-        if (int rc = do_bc(h, chain[s], st)) return rc;
+        if (int rc = do_bc(h, src, st)) return rc;
       RkArgs rk;
-      rk_coefficients(s, &rk.A, &rk.B);
-      rk.dt = dt; rk.Qtmp = Qtmp; rk.Qout = chain[s + 1]; rk.first = (s == 0); rk.wrap = wrap ? 1 : 0;
-      if (int rc = do_rhs(h, chain[s], h->R, &rk, st)) return rc;
+      rk_coefficients(nstages, s, &rk.A, &rk.B);
+      rk.dt = dt; rk.Qtmp = Qtmp; rk.Qout = dst; rk.first = (s == 0); rk.wrap = wrap ? 1 : 0;
+      if (int rc = do_rhs(h, src, h->R, &rk, st)) return rc;
     } else {
       if (int rc = do_bc(h, Q, st)) return rc;
       if (int rc = do_rhs(h, Q, h->R, nullptr, st)) return rc;
-      OSBLI_LAUNCH(h, OSBLI_K_RK, st, launch_rk_update(h->P, s, dt, Q, Qtmp, h->R, st));
+      OSBLI_LAUNCH(h, OSBLI_K_RK, st, launch_rk_update(h->P, nstages, s, dt, Q, Qtmp, h->R, st));
     }
   }
   return wrap ? OSBLI_OK : do_bc(h, Q, st);
@@ -258,7 +259,12 @@ int osbli_rhs(osbli_handle h, const double *d_Q, double *d_R, void *cuda_stream)
 
 int osbli_rk3_step(osbli_handle h, double *d_Q, double *d_Qtmp, double dt, void *cuda_stream) {
   if (!h || !d_Q || !d_Qtmp || d_Q == d_Qtmp) return OSBLI_EINVAL;
-  return do_step(h, d_Q, d_Qtmp, dt, as_stream(cuda_stream));
+  return do_step(h, 3, d_Q, d_Qtmp, dt, as_stream(cuda_stream));
+}
+
+int osbli_rk4_step(osbli_handle h, double *d_Q, double *d_Qtmp, double dt, void *cuda_stream) {
+  if (!h || !d_Q || !d_Qtmp || d_Q == d_Qtmp) return OSBLI_EINVAL;
+  return do_step(h, 5, d_Q, d_Qtmp, dt, as_stream(cuda_stream));
 }
 
 int osbli_advance_host(osbli_handle h, double *h_Q, double *d_Q, double *d_Qtmp, double dt, int32_t nsteps,
@@ -268,7 +274,7 @@ int osbli_advance_host(osbli_handle h, double *h_Q, double *d_Q, double *d_Qtmp,
   const size_t bytes = (size_t)5 * (size_t)h->P.L.sv * sizeof(double);
   if (cudaMemcpyAsync(d_Q, h_Q, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return OSBLI_ECUDA;
   for (int s = 0; s < nsteps; ++s)
-    if (int rc = do_step(h, d_Q, d_Qtmp, dt, st)) return rc;
+    if (int rc = do_step(h, 3, d_Q, d_Qtmp, dt, st)) return rc;
   if (cudaMemcpyAsync(h_Q, d_Q, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return OSBLI_ECUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return OSBLI_ECUDA;
   return OSBLI_OK;

@@ -163,21 +163,29 @@ rk_update_kernel(const __grid_constant__ DevParams P, double A, double B, double
   }
 }
 
-void rk_coefficients(int stage, double *A, double *B) {
-  const double a[3] = {0.0, -5.0 / 9.0, -153.0 / 128.0};
-  const double b[3] = {1.0 / 3.0, 15.0 / 16.0, 8.0 / 15.0};
-  *A = a[stage]; *B = b[stage];
+// Coefficients of eq. (36)-(37) "from [23]": nstages = 3 -> Williamson's 2N-storage RK3
+// (Q15); nstages = 5 -> Carpenter & Kennedy's five-stage 4th-order 2N-storage scheme (Q35).
+void rk_coefficients(int nstages, int stage, double *A, double *B) {
+  static const double a3[3] = {0.0, -5.0 / 9.0, -153.0 / 128.0};
+  static const double b3[3] = {1.0 / 3.0, 15.0 / 16.0, 8.0 / 15.0};
+  static const double a5[5] = {0.0, -567301805773.0 / 1357537059087.0, -2404267990393.0 / 2016746695238.0,
+                               -3550918686646.0 / 2091501179385.0, -1275806237668.0 / 842570457699.0};
+  static const double b5[5] = {1432997174477.0 / 9575080441755.0, 5161836677717.0 / 13612068292357.0,
+                               1720146321549.0 / 2090206949498.0, 3134564353537.0 / 4481467310338.0,
+                               2277821191437.0 / 14882151754819.0};
+  *A = nstages == 5 ? a5[stage] : a3[stage];
+  *B = nstages == 5 ? b5[stage] : b3[stage];
 }
 
-cudaError_t launch_rk_update(const DevParams &P, int stage, double dt, double *Q, double *Qtmp, const double *R,
-                             cudaStream_t st) {
-  double A[3], B[3];
-  for (int s = 0; s < 3; ++s) rk_coefficients(s, &A[s], &B[s]);
+cudaError_t launch_rk_update(const DevParams &P, int nstages, int stage, double dt, double *Q, double *Qtmp,
+                             const double *R, cudaStream_t st) {
+  double A, B;
+  rk_coefficients(nstages, stage, &A, &B);
   const Layout &L = P.L;
   const int pairs = (L.n[0] + 1) / 2;
   dim3 grid((pairs + 127) / 128, L.n[1], L.n[2]);
-  if (stage == 0) rk_update_kernel<true><<<grid, 128, 0, st>>>(P, A[0], B[0], dt, Q, Qtmp, R);
-  else rk_update_kernel<false><<<grid, 128, 0, st>>>(P, A[stage], B[stage], dt, Q, Qtmp, R);
+  if (stage == 0) rk_update_kernel<true><<<grid, 128, 0, st>>>(P, A, B, dt, Q, Qtmp, R);
+  else rk_update_kernel<false><<<grid, 128, 0, st>>>(P, A, B, dt, Q, Qtmp, R);
   return cudaGetLastError();
 }
 

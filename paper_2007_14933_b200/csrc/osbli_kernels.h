@@ -9,7 +9,7 @@ namespace osbli {
 // wrap != 0 (all active directions periodic): the periodic images of the boundary-near nodes are
 // written into the halos of Qout as well, which replaces the halo fill of the next stage.
 struct RkArgs { double A, B, dt; double *Qtmp, *Qout; int first, wrap; };
-void rk_coefficients(int stage, double *A, double *B);
+void rk_coefficients(int nstages, int stage, double *A, double *B);   // nstages = 3 (RK3) or 5 (RK4)
 
 // R (-)= flux difference of the characteristic reconstruction along `dir` (osbli_sweep.cu).
 // rk != nullptr (dir 1 or 2, accumulate = 1 only): R is read but not written, the stage update is done instead.
@@ -31,7 +31,7 @@ cudaError_t launch_force(const DevParams &P, const double *Q, double *R, cudaStr
 cudaError_t launch_bc(const DevParams &P, int dir, double *Q, cudaStream_t st);
 
 // RK3 stage update, eq. (36)-(37): Qtmp = A Qtmp + dt R; Q += B Qtmp on interior nodes
-cudaError_t launch_rk_update(const DevParams &P, int stage, double dt, double *Q, double *Qtmp, const double *R, cudaStream_t st);
+cudaError_t launch_rk_update(const DevParams &P, int nstages, int stage, double dt, double *Q, double *Qtmp, const double *R, cudaStream_t st);
 
 // DFMA micro-benchmark (osbli_peak.cu): measured fp64 TFLOP/s of this device; d_scratch >= 8 bytes
 cudaError_t measure_fp64_peak(double *d_scratch, cudaStream_t st, double *tflops);

@@ -71,6 +71,8 @@ _lib.osbli_rhs.restype = C.c_int
 _lib.osbli_rhs.argtypes = [_h, _dp, _dp, _dp]
 _lib.osbli_rk3_step.restype = C.c_int
 _lib.osbli_rk3_step.argtypes = [_h, _dp, _dp, C.c_double, _dp]
+_lib.osbli_rk4_step.restype = C.c_int
+_lib.osbli_rk4_step.argtypes = [_h, _dp, _dp, C.c_double, _dp]
 _lib.osbli_advance_host.restype = C.c_int
 _lib.osbli_advance_host.argtypes = [_h, _dp, _dp, _dp, C.c_double, C.c_int32, _dp]
 _lib.osbli_launch_count.restype = C.c_int
@@ -87,7 +89,7 @@ _lib.osbli_strerror.restype = C.c_char_p
 _lib.osbli_strerror.argtypes = [C.c_int]
 
 EXPORTS = ("osbli_get_layout", "osbli_workspace_bytes", "osbli_init", "osbli_bc", "osbli_rhs",
-           "osbli_rk3_step", "osbli_advance_host", "osbli_launch_count", "osbli_profile_begin", "osbli_profile_end",
+           "osbli_rk3_step", "osbli_rk4_step", "osbli_advance_host", "osbli_launch_count", "osbli_profile_begin", "osbli_profile_end",
            "osbli_measure_fp64_peak", "osbli_destroy", "osbli_strerror")
 K_CLASSES = ("bc", "primitives", "sweep_x", "sweep_y", "sweep_z", "viscous", "rk_update")
 
@@ -136,6 +138,10 @@ def osbli_rhs(handle, q_ptr, r_ptr, stream=0):
 
 def osbli_rk3_step(handle, q_ptr, qtmp_ptr, dt, stream=0):
     _check(_lib.osbli_rk3_step(handle, q_ptr, qtmp_ptr, float(dt), stream), "osbli_rk3_step")
+
+
+def osbli_rk4_step(handle, q_ptr, qtmp_ptr, dt, stream=0):
+    _check(_lib.osbli_rk4_step(handle, q_ptr, qtmp_ptr, float(dt), stream), "osbli_rk4_step")
 
 
 def osbli_advance_host(handle, hq_ptr, q_ptr, qtmp_ptr, dt, nsteps, stream=0):
@@ -267,6 +273,10 @@ class Solver:
 
     def rk3_step(self, Q, Qtmp, dt):
         osbli_rk3_step(self.handle, Q.data_ptr(), Qtmp.data_ptr(), dt, self._stream())
+        return Q
+
+    def rk4_step(self, Q, Qtmp, dt):
+        osbli_rk4_step(self.handle, Q.data_ptr(), Qtmp.data_ptr(), dt, self._stream())
         return Q
 
     def advance_host(self, hQ, Q, Qtmp, dt, nsteps):

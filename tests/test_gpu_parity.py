@@ -132,15 +132,15 @@ def test_residual_curvilinear_3d_periodic_const_visc():
 
 
 # ----------------------------------------------------------------------------- RK3 steps ----
-def run_steps_case(name, case, nsteps, tol, norm, **over):
+def run_steps_case(name, case, nsteps, tol, norm, rk4=False, **over):
     metrics = parity.metrics_for(case)
     orc = parity.make_oracle(case, metrics, **over)
     sol = parity.make_solver(case, metrics, **over)
-    Qo = orc.run(case.Q0.copy(), case.dt, nsteps)
+    Qo = orc.run(case.Q0.copy(), case.dt, nsteps, rk4=rk4)
     Q = sol.to_padded(case.Q0)
     Qtmp = sol.empty_state()
     for _ in range(nsteps):
-        sol.rk3_step(Q, Qtmp, case.dt)
+        (sol.rk4_step if rk4 else sol.rk3_step)(Q, Qtmp, case.dt)
     _torch().cuda.synchronize()
     Qg = sol.from_padded(Q)
     a, b = parity.interior(case, Qg), parity.interior(case, Qo)
@@ -251,6 +251,14 @@ def test_channel_adiabatic_wall_and_body_force():
     run_residual_case("channel3d_teno5", W.channel(n=(24, 33, 6), noise=1e-3, scheme=W.TENO5))
     run_steps_case("channel_20", case, 20, 1e-9, parity.q28)
     run_steps_case("channel3d_5", W.channel(n=(24, 33, 6), noise=1e-3, scheme=W.TENO5), 5, 1e-9, parity.q28)
+
+
+def test_steps_rk4_five_stage():
+    """the five-stage 4th-order member of the low-storage family (osbli_rk4_step): fused
+    path with periodic write-through (Q -> Q2 -> Q3 -> Q2 -> Q3 -> Q), fused path with halo-fill passes, 1-D path."""
+    run_steps_case("tgv32_5_rk4", W.tgv(32), 5, 1e-9, parity.q28, rk4=True)
+    run_steps_case("wavy_box_3_rk4", W.wavy_box(n=(40, 21, 9)), 3, 1e-9, parity.l1_rel, rk4=True)
+    run_steps_case("sod_200_rk4", W.sod(), 200, 1e-9, parity.l1_rel, rk4=True)
 
 
 def test_advance_host_matches_device_steps():
