@@ -635,6 +635,7 @@ int validate(const oracle_params *p) {
     if ((p->bc[d][0] == ORACLE_BC_PERIODIC) != (p->bc[d][1] == ORACLE_BC_PERIODIC)) return 1;
   }
   if (p->nthreads < 1) return 1;
+  if (p->scheme == ORACLE_CENTRAL4 && p->curvilinear) return 1;   /* central convective terms: uniform grids only */
   return 0;
 }
 
@@ -744,6 +745,33 @@ void rhs_full(const oracle_params *p, const Grid &g, const double *Q, double *R,
           int ijk[3];
           ijk[d] = 0; ijk[e1] = b; ijk[e2] = a;
           const long base = g.idx(ijk[0], ijk[1], ijk[2]);
+          if (p->scheme == ORACLE_CENTRAL4) {
+            /* "Central schemes are also applied to smooth problems that do not require shock-capturing"
+             * (PAPER.md:198): the convective terms as the 4th-order central difference eq. (28) of the
+             * point-wise flux vectors (one-sided closures eq. (30)-(33) next to non-periodic boundaries);
+             * uniform grids only (Q36). */
+            for (int i = 0; i < n; ++i) {
+              double cf[5];
+              const int off = d1_coeffs(n, i, p->bc[d][0] == ORACLE_BC_PERIODIC, cf);
+              double acc[5] = {0, 0, 0, 0, 0};
+              for (int m = 0; m < 5; ++m) {
+                if (cf[m] == 0.0) continue;
+                double q[5], f[5];
+                load_state(g, Q, base + (long)(i + off + m) * s, q);
+                const Prim w = prim_of(p, q);
+                const double th = d == 0 ? w.u : (d == 1 ? w.v : w.w);
+                f[0] = q[0] * th;
+                f[1] = q[1] * th + (d == 0 ? w.p : 0.0);
+                f[2] = q[2] * th + (d == 1 ? w.p : 0.0);
+                f[3] = q[3] * th + (d == 2 ? w.p : 0.0);
+                f[4] = (q[4] + w.p) * th;
+                for (int c = 0; c < 5; ++c) acc[c] += cf[m] * f[c];
+              }
+              const long at = base + (long)i * s;
+              for (int c = 0; c < 5; ++c) R[c * g.total + at] -= acc[c] / (12.0 * p->delta[d]);
+            }
+            continue;
+          }
           /* step 2: every half node of this line, -1/2 ... n-1/2 */
           std::vector<double> fh((size_t)(n + 1) * 5), mg((size_t)n + 1);
           for (int q = 0; q <= n; ++q)
@@ -854,6 +882,7 @@ int32_t oracle_rhs(const oracle_params *p, const double *Q, double *R, int32_t p
 int32_t oracle_rhs_points(const oracle_params *p, const double *Q, int32_t parts,
                           int64_t npts, const int32_t *ijk, double *out) {
   if (validate(p)) return 1;
+  if (p->scheme == ORACLE_CENTRAL4) return 2;          /* node-by-node evaluation exists for the reconstruction schemes only */
   const Grid g = make_grid(p);
   PrimSource ps{p, &g, Q, nullptr};
 #pragma omp parallel for num_threads(p->nthreads) schedule(dynamic, 16)
