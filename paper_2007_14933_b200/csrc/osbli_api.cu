@@ -50,7 +50,8 @@ int validate(const osbli_params *p) {
   Layout L;
   if (int rc = make_layout(p, &L)) return rc;
   if (p->nx == 1) return OSBLI_EUNSUPPORTED;                       // x is the contiguous direction; it must be active
-  if (p->scheme < OSBLI_SCHEME_WENOZ5 || p->scheme > OSBLI_SCHEME_WENOJS5) return OSBLI_EINVAL;
+  if (p->scheme < OSBLI_SCHEME_WENOZ5 || p->scheme > OSBLI_SCHEME_CENTRAL4) return OSBLI_EINVAL;
+  if (p->scheme == OSBLI_SCHEME_CENTRAL4 && p->metrics) return OSBLI_EUNSUPPORTED;   // central convective terms: uniform grids
   if (p->visc < OSBLI_VISC_NONE || p->visc > OSBLI_VISC_SUTHERLAND) return OSBLI_EINVAL;
   if (!(p->gamma > 1.0)) return OSBLI_EINVAL;
   if (!(p->eps >= 1e-18) || !(p->teno_ct > 0.0)) return OSBLI_EINVAL;
@@ -117,6 +118,14 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
   const DevParams &P = h->P;
   const bool fast_visc = viscous_fast_path(P);
   if (P.visc != OSBLI_VISC_NONE && !fast_visc) OSBLI_LAUNCH(h, OSBLI_K_PRIM, st, launch_primitives(P, Q, h->prim, st));
+  if (P.scheme == OSBLI_SCHEME_CENTRAL4) {                            // no sweeps: central convective terms, then the rest
+    if (rk) return OSBLI_EINVAL;
+    OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X, st, launch_central(P, Q, R, st));
+    if (fast_visc) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous_fast(P, Q, R, st));
+    else if (P.visc != OSBLI_VISC_NONE) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, 1, st));
+    if (P.has_force) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_force(P, Q, R, st));
+    return OSBLI_OK;
+  }
   int last = 0;
   for (int d = 0; d < 3; ++d)
     if (P.L.n[d] > 1) last = d;
@@ -142,7 +151,7 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
 // so the state moves Q -> Q2 -> Q3 (-> Q2 -> Q3) -> Q through two workspace states; 1-D problems use the
 // separate in-place update kernel.  The result is in Q either way.
 int do_step(osbli_ctx *h, int nstages, double *Q, double *Qtmp, double dt, cudaStream_t st) {
-  const bool fuse = h->P.L.n[1] > 1 || h->P.L.n[2] > 1;
+  const bool fuse = (h->P.L.n[1] > 1 || h->P.L.n[2] > 1) && h->P.scheme != OSBLI_SCHEME_CENTRAL4;
   bool wrap = fuse;                  // every active direction periodic: the fused update fills the halos itself
   for (int d = 0; d < 3; ++d)
     if (h->P.L.n[d] > 1 && !h->P.periodic[d]) wrap = false;

@@ -24,6 +24,9 @@ cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *pr
 bool viscous_fast_path(const DevParams &P);
 cudaError_t launch_viscous_fast(const DevParams &P, const double *Q, double *R, cudaStream_t st);
 
+// central convective terms, scheme 4 (osbli_visc.cu): R = - sum_d delta_d F_d on interior nodes (writes R)
+cudaError_t launch_central(const DevParams &P, const double *Q, double *R, cudaStream_t st);
+
 // constant body force (osbli_bc_rk.cu): R_{rho u_i} += f_i, R_{rho E} += u_i f_i on interior nodes
 cudaError_t launch_force(const DevParams &P, const double *Q, double *R, cudaStream_t st);
 

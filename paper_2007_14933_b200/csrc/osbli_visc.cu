@@ -221,6 +221,57 @@ viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ p
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Central convective terms (scheme 4, uniform grids): R = - sum_d delta_d F_d with the 4th-order
+// first difference eq. (28) (closures eq. (30)-(33) next to non-periodic boundaries) of the point-wise
+// flux vectors.  One thread per node, x fastest: every neighbour access of a warp
+// is a contiguous row segment; the 12 neighbours are shared with the adjacent threads / rows through
+// L1 and L2.  First kernel of the stage: writes all five components of R.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+central_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R) {
+  const Layout &L = P.L;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= L.n[0]) return;
+  const int nd[3] = {i, (int)blockIdx.y, (int)blockIdx.z};
+  const long long at = L.at(nd[0], nd[1], nd[2]);
+  const long long sv = L.sv;
+  const long long st[3] = {1, L.sy, L.sz};
+  double acc[5] = {0, 0, 0, 0, 0};
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    if (L.n[d] <= 1) continue;
+    double c[5];
+    const int o = d1_stencil(L.n[d], nd[d], P.periodic[d], c);
+    const double s = P.inv12d[d];
+#pragma unroll
+    for (int m = 0; m < 5; ++m) {
+      if (c[m] == 0.0) continue;
+      const long long a = at + (long long)(o + m) * st[d];
+      const double r = __ldg(Q + a), mx = __ldg(Q + sv + a), my = __ldg(Q + 2 * sv + a), mz = __ldg(Q + 3 * sv + a);
+      const double E = __ldg(Q + 4 * sv + a);
+      const double ir = 1.0 / r;
+      const double p = P.gm1 * (E - 0.5 * ir * (mx * mx + my * my + mz * mz));
+      const double th = (d == 0 ? mx : (d == 1 ? my : mz)) * ir;
+      const double w = c[m] * s;
+      acc[0] = fma(w, r * th, acc[0]);
+      acc[1] = fma(w, mx * th + (d == 0 ? p : 0.0), acc[1]);
+      acc[2] = fma(w, my * th + (d == 1 ? p : 0.0), acc[2]);
+      acc[3] = fma(w, mz * th + (d == 2 ? p : 0.0), acc[3]);
+      acc[4] = fma(w, (E + p) * th, acc[4]);
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 5; ++c) R[c * sv + at] = -acc[c];
+}
+
+cudaError_t launch_central(const DevParams &P, const double *Q, double *R, cudaStream_t st) {
+  const Layout &L = P.L;
+  dim3 grid((L.n[0] + 127) / 128, L.n[1], L.n[2]);
+  central_kernel<<<grid, 128, 0, st>>>(P, Q, R);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_primitives(const DevParams &P, const double *Q, double *prim, cudaStream_t st) {
   const Layout &L = P.L;
   const int NX = L.n[0] + 2 * L.h[0];

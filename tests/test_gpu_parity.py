@@ -261,6 +261,30 @@ def test_steps_rk4_five_stage():
     run_steps_case("sod_200_rk4", W.sod(), 200, 1e-9, parity.l1_rel, rk4=True)
 
 
+def test_central4_scheme():
+    """SURVEY.md 8(f) NEXT-4 (first step): 4th-order central convective terms (scheme 4) with the central
+    viscous terms, unfused update: periodic 3-D (fast viscous path), ragged sizes, non-periodic 2-D box
+    (closures), 1-D, and through the RK3 / RK4 steps."""
+    case = W.tgv(32, scheme=W.CENTRAL4)
+    run_residual_case("tgv32_central", case)
+    run_residual_case("tgv32_central_perturbed_euler", case, Q0=W.perturb(case, seed=5, amp=0.05), visc=W.VISC_NONE)
+    run_residual_case("pbox_central_70x37x35", _periodic_box((70, 37, 35), scheme=W.CENTRAL4))
+    n = (40, 33, 1)
+    i, j, k = W.padded_index_grids(n)
+    x, y = i / (n[0] - 1.0) + 0 * j + 0 * k, j / (n[1] - 1.0) + 0 * i + 0 * k
+    g, M = 1.4, 0.8
+    Q0 = np.ascontiguousarray(W.conservative(1.0 + 0.1 * np.sin(3 * x) * np.cos(2 * y), 0.5 + 0.2 * np.sin(2 * x + y),
+                                             0.1 * np.cos(3 * x - 2 * y), 0.0, (1.0 + 0.1 * np.cos(2 * x + 3 * y)) / (g * M * M), g))
+    ex = (W.BC_EXTRAP0, W.BC_EXTRAP0)
+    box = W.Case(name="box2d", n=n, Q0=Q0, dt=1e-3, nsteps=1, delta=(1.0 / (n[0] - 1), 1.0 / (n[1] - 1), 1.0), gamma=g,
+                 Re=200.0, Pr=0.72, Minf=M, scheme=W.CENTRAL4, visc=W.VISC_SUTHERLAND, bc=(ex, ex, (0, 0)))
+    run_residual_case("box2d_central_sutherland", box)
+    run_residual_case("sod_central", W.sod(scheme=W.CENTRAL4))
+    run_steps_case("tgv32_10_central", case, 10, 1e-9, parity.q28)
+    run_steps_case("tgv32_4_central_rk4", case, 4, 1e-9, parity.q28, rk4=True)
+    run_steps_case("channel_central_10", W.channel(n=(32, 64, 1), noise=1e-3, scheme=W.CENTRAL4), 10, 1e-9, parity.q28)
+
+
 def test_advance_host_matches_device_steps():
     case = W.tgv(32)
     sol = parity.make_solver(case)
