@@ -373,7 +373,9 @@ static cudaError_t launch_yz(const DevParams &P, const double *Q, double *R, int
   const int n = P.L.n[DIR];
   const int nt = (DIR == 1) ? P.L.n[2] : P.L.n[1];
   const int bx = nx >= 128 ? 128 : (nx > 64 ? 128 : (nx > 32 ? 64 : 32));
+  // segments of 64 nodes (6 warm-up nodes each) where that still leaves >= 4 waves of blocks, else 32
   int chunk = n > 64 ? 32 : n;
+  if (n > 64 && (long long)((nx + bx - 1) / bx) * nt * ((n + 63) / 64) >= 4LL * 2 * 148) chunk = 64;
   dim3 grid((nx + bx - 1) / bx, nt, (n + chunk - 1) / chunk);
   const RkArgs none = {0.0, 0.0, 0.0, nullptr, nullptr, 0, 0};
   if (rk) {
