@@ -136,9 +136,11 @@ int osbli_rk3_step(osbli_handle h, double *d_Q, double *d_Qtmp, double dt, void 
  * 4th order schemes have three and five sub-stages per iteration"): Q -> Q2 -> Q3 -> Q2 -> Q3 -> Q. */
 int osbli_rk4_step(osbli_handle h, double *d_Q, double *d_Qtmp, double dt, void *cuda_stream);
 
-/* End-to-end convenience with HOST buffers: copies h_Q (host, padded layout, total_doubles
- * doubles) to d_Q, runs nsteps RK3 steps of size dt, copies the state back into h_Q and
- * synchronises the stream.  d_Q, d_Qtmp: device scratch states owned by the caller. */
+/* End-to-end convenience with HOST buffers: copies the interior nodes of h_Q (host, padded layout,
+ * total_doubles doubles) to d_Q, runs nsteps RK3 steps of size dt (halos are rebuilt on the device),
+ * copies the interior nodes of the result back into h_Q and synchronises the stream.  Halo and padding
+ * entries of h_Q are neither read nor written (5 * nx * ny * nz doubles cross the bus each way).
+ * d_Q, d_Qtmp: device scratch states owned by the caller. */
 int osbli_advance_host(osbli_handle h, double *h_Q, double *d_Q, double *d_Qtmp, double dt,
                        int32_t nsteps, void *cuda_stream);
 
