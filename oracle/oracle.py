@@ -19,7 +19,7 @@ _SRC = _HERE / "osbli_oracle.cpp"
 _HDR = _HERE / "osbli_oracle.h"
 _LIB = _HERE / "libosbli_oracle.so"
 
-WENOZ5, TENO5, TENO6, WENOJS5, CENTRAL4 = 0, 1, 2, 3, 4
+WENOZ5, TENO5, TENO6, WENOJS5, CENTRAL4, WENOZ3 = 0, 1, 2, 3, 4, 5
 VISC_NONE, VISC_CONST, VISC_SUTHERLAND = 0, 1, 2
 BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL = 0, 1, 2, 3
 PART_INVISCID, PART_VISCOUS = 1, 2

@@ -97,6 +97,19 @@ double reconstruct(int scheme, double a, double b, double c, double d, double e,
 
   if (margin) *margin = std::numeric_limits<double>::infinity();
 
+  if (scheme == ORACLE_WENOZ3) {
+    /* Third-order WENO-Z (k = 2 in the notation of PAPER.md:147-167): two 2-point candidates
+     * q_0 = (c + d)/2 on {c,d}, q_1 = (-b + 3c)/2 on {b,c}; ideal weights 2/3, 1/3 (their combination is the
+     * 3rd-order value (-b + 5c + 2d)/6); Jiang-Shu indicators of the linear candidates beta_0 = (d - c)^2,
+     * beta_1 = (c - b)^2; tau = |beta_0 - beta_1|; weights eq. (22) (Q37). */
+    const double q0 = 0.5 * (c + d), q1 = 0.5 * (-b + 3.0 * c);
+    const double be0 = (d - c) * (d - c), be1 = (c - b) * (c - b);
+    const double tau3 = std::fabs(be0 - be1);
+    const double r0 = tau3 / (be0 + eps), r1 = tau3 / (be1 + eps);
+    const double a0 = 2.0 / 3.0 * (1.0 + r0 * r0), a1 = 1.0 / 3.0 * (1.0 + r1 * r1);
+    return a0 / (a0 + a1) * q0 + a1 / (a0 + a1) * q1;
+  }
+
   if (scheme == ORACLE_WENOJS5) {
     /* eq. (20)-(21): alpha_r = d_r / (eps + beta_r)^p, p = 2 (eps = 1e-6 there) */
     const double aR = dR / ((eps + bR) * (eps + bR));

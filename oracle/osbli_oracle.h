@@ -31,7 +31,8 @@
 extern "C" {
 #endif
 
-enum { ORACLE_WENOZ5 = 0, ORACLE_TENO5 = 1, ORACLE_TENO6 = 2, ORACLE_WENOJS5 = 3, ORACLE_CENTRAL4 = 4 };
+enum { ORACLE_WENOZ5 = 0, ORACLE_TENO5 = 1, ORACLE_TENO6 = 2, ORACLE_WENOJS5 = 3, ORACLE_CENTRAL4 = 4,
+       ORACLE_WENOZ3 = 5 };
 enum { ORACLE_VISC_NONE = 0, ORACLE_VISC_CONST = 1, ORACLE_VISC_SUTHERLAND = 2 };
 enum { ORACLE_BC_PERIODIC = 0, ORACLE_BC_EXTRAP0 = 1, ORACLE_BC_DIRICHLET = 2, ORACLE_BC_WALL_ISOTHERMAL = 3,
        ORACLE_BC_WALL_ADIABATIC = 4 };

@@ -20,7 +20,7 @@ from typing import Optional
 
 import numpy as np
 
-WENOZ5, TENO5, TENO6, WENOJS5, CENTRAL4 = 0, 1, 2, 3, 4
+WENOZ5, TENO5, TENO6, WENOJS5, CENTRAL4, WENOZ3 = 0, 1, 2, 3, 4, 5
 VISC_NONE, VISC_CONST, VISC_SUTHERLAND = 0, 1, 2
 BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL, BC_WALL_ADIABATIC = 0, 1, 2, 3, 4
 

@@ -30,6 +30,12 @@ def prim(Q):
 def weights_and_value(pts, scheme, eps=1e-16, ct=1e-6):
     """pts: the stencil values [a, b, c, d, e(, f)], upwind side a, b, c; interface between c and d."""
     a, b, c, d, e = pts[:5]
+    if scheme == W.WENOZ3:                                  # k = 2: two linear candidates, weights eq. (22)
+        q3 = [(c + d) / 2, (-b + 3 * c) / 2]
+        be = [(d - c) ** 2, (c - b) ** 2]
+        t3 = np.abs(be[0] - be[1])
+        al3 = [2 / 3 * (1 + (t3 / (be[0] + eps)) ** 2), 1 / 3 * (1 + (t3 / (be[1] + eps)) ** 2)]
+        return (al3[0] * q3[0] + al3[1] * q3[1]) / (al3[0] + al3[1])
     q = [(2 * c + 5 * d - e) / 6, (-b + 5 * c + 2 * d) / 6, (2 * a - 7 * b + 11 * c) / 6]
     beta = [13 / 12 * (c - 2 * d + e) ** 2 + (3 * c - 4 * d + e) ** 2 / 4,
             13 / 12 * (b - 2 * c + d) ** 2 + (b - d) ** 2 / 4,
@@ -181,7 +187,7 @@ def box(n, seed):
                   delta=tuple(2 * np.pi / v_ for v_ in n), gamma=G, Re=50.0, Pr=0.71, Minf=0.7, bc=bc)
 
 
-@pytest.mark.parametrize("scheme", [W.WENOZ5, W.TENO5, W.TENO6, W.WENOJS5, W.CENTRAL4])
+@pytest.mark.parametrize("scheme", [W.WENOZ5, W.TENO5, W.TENO6, W.WENOJS5, W.CENTRAL4, W.WENOZ3])
 @pytest.mark.parametrize("n", [(8, 6, 5), (12, 10, 1), (16, 1, 1)])
 @pytest.mark.parametrize("visc", [W.VISC_NONE, W.VISC_CONST])
 def test_p12_oracle_equals_vectorised_numpy(scheme, n, visc):
