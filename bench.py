@@ -32,7 +32,8 @@ UNIT = "updates/s"
 FLOP_SWEEP = {0: 1256 + 15 + 19, 1: 1356 + 15 + 19,      # WENO-Z5, TENO5: interface + difference + primitives
               2: 1856 + 15 + 19,                          # TENO6: + ~50 per reconstruction (hand count)
               3: 1206 + 15 + 19,                          # WENO-JS5: WENO-Z5 minus tau and the (1 + (.)^2) factors
-              4: 90}                                      # central4: 4 stencil points x ~17 flop + combination, per direction
+              4: 90,                                      # central4: 4 stencil points x ~17 flop + combination, per direction
+              5: 900}                                     # WENO-Z3: projections as for the 5-point schemes, ~25 per reconstruction
 FLOP_VISCOUS = 300
 FLOP_RK = 20
 
@@ -207,7 +208,7 @@ def run_ours(args):
 
     n = args.n
     scheme = {"wenoz5": W.WENOZ5, "teno5": W.TENO5, "teno6": W.TENO6, "wenojs5": W.WENOJS5,
-              "central4": W.CENTRAL4}[args.scheme]
+              "central4": W.CENTRAL4, "wenoz3": W.WENOZ3}[args.scheme]
     case = W.tgv(n, scheme=scheme)
     if scheme == W.WENOJS5:
         case.eps = 1e-6                                   # eq. (21)
@@ -340,7 +341,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=256, help="grid points per side (256 = BASELINE.json config 3)")
-    ap.add_argument("--scheme", default="teno5", choices=["wenoz5", "teno5", "teno6", "wenojs5", "central4"],
+    ap.add_argument("--scheme", default="teno5", choices=["wenoz5", "teno5", "teno6", "wenojs5", "central4", "wenoz3"],
                     help="reconstruction (teno5 = BASELINE.json config 3; the others are side measurements)")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -47,7 +47,8 @@ typedef struct osbli_ctx *osbli_handle;
 enum { OSBLI_OK = 0, OSBLI_EINVAL = 1, OSBLI_EUNSUPPORTED = 2, OSBLI_ECUDA = 3, OSBLI_EWORKSPACE = 4 };
 enum { OSBLI_SCHEME_WENOZ5 = 0, OSBLI_SCHEME_TENO5 = 1, OSBLI_SCHEME_TENO6 = 2,
        OSBLI_SCHEME_WENOJS5 = 3 /* eq. (20)-(21); set eps = 1e-6 */,
-       OSBLI_SCHEME_CENTRAL4 = 4 /* eq. (28) on the flux vectors, no shock capturing; uniform grids */ };
+       OSBLI_SCHEME_CENTRAL4 = 4 /* eq. (28) on the flux vectors, no shock capturing; uniform grids */,
+       OSBLI_SCHEME_WENOZ3 = 5 /* third-order WENO-Z */ };
 enum { OSBLI_VISC_NONE = 0 /* Euler */, OSBLI_VISC_CONST = 1 /* mu = 1 */,
        OSBLI_VISC_SUTHERLAND = 2 /* PAPER.md:59-63, 317-318 */ };
 enum { OSBLI_BC_PERIODIC = 0, OSBLI_BC_EXTRAP0 = 1, OSBLI_BC_DIRICHLET = 2,

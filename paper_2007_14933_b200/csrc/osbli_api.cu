@@ -50,7 +50,7 @@ int validate(const osbli_params *p) {
   Layout L;
   if (int rc = make_layout(p, &L)) return rc;
   if (p->nx == 1) return OSBLI_EUNSUPPORTED;                       // x is the contiguous direction; it must be active
-  if (p->scheme < OSBLI_SCHEME_WENOZ5 || p->scheme > OSBLI_SCHEME_CENTRAL4) return OSBLI_EINVAL;
+  if (p->scheme < OSBLI_SCHEME_WENOZ5 || p->scheme > OSBLI_SCHEME_WENOZ3) return OSBLI_EINVAL;
   if (p->scheme == OSBLI_SCHEME_CENTRAL4 && p->metrics) return OSBLI_EUNSUPPORTED;   // central convective terms: uniform grids
   if (p->visc < OSBLI_VISC_NONE || p->visc > OSBLI_VISC_SUTHERLAND) return OSBLI_EINVAL;
   if (!(p->gamma > 1.0)) return OSBLI_EINVAL;

@@ -406,6 +406,8 @@ cudaError_t launch_sweep(const DevParams &P, int dir, const double *Q, double *R
   OSBLI_DISPATCH(2, true)
   OSBLI_DISPATCH(3, false)
   OSBLI_DISPATCH(3, true)
+  OSBLI_DISPATCH(5, false)
+  OSBLI_DISPATCH(5, true)
 #undef OSBLI_DISPATCH
   return cudaErrorInvalidValue;
 }

@@ -25,7 +25,7 @@ if not _LIBPATH.exists():
 _lib = C.CDLL(str(_LIBPATH))
 
 OK, EINVAL, EUNSUPPORTED, ECUDA, EWORKSPACE = 0, 1, 2, 3, 4
-SCHEME_WENOZ5, SCHEME_TENO5, SCHEME_TENO6, SCHEME_WENOJS5, SCHEME_CENTRAL4 = 0, 1, 2, 3, 4
+SCHEME_WENOZ5, SCHEME_TENO5, SCHEME_TENO6, SCHEME_WENOJS5, SCHEME_CENTRAL4, SCHEME_WENOZ3 = 0, 1, 2, 3, 4, 5
 VISC_NONE, VISC_CONST, VISC_SUTHERLAND = 0, 1, 2
 BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL, BC_WALL_ADIABATIC = 0, 1, 2, 3, 4
 

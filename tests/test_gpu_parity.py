@@ -285,6 +285,18 @@ def test_central4_scheme():
     run_steps_case("channel_central_10", W.channel(n=(32, 64, 1), noise=1e-3, scheme=W.CENTRAL4), 10, 1e-9, parity.q28)
 
 
+def test_wenoz3_scheme():
+    """third-order WENO-Z (scheme 5) on the same kernels."""
+    case = W.tgv(32, scheme=W.WENOZ3)
+    run_residual_case("tgv32_wenoz3_perturbed", case, Q0=W.perturb(case, seed=5, amp=0.05))
+    run_residual_case("wavy_box_wenoz3", W.wavy_box(n=(24, 20, 8), scheme=W.WENOZ3))
+    sod = W.sod(scheme=W.WENOZ3)
+    orc = parity.make_oracle(sod)
+    run_residual_case("sod_t0.03_wenoz3", sod, Q0=orc.run(sod.Q0.copy(), sod.dt, 150))
+    run_steps_case("tgv32_10_wenoz3", case, 10, 1e-9, parity.q28)
+    run_steps_case("sod_300_wenoz3", sod, 300, 1e-9, parity.l1_rel)
+
+
 def test_advance_host_matches_device_steps():
     case = W.tgv(32)
     sol = parity.make_solver(case)
