@@ -58,7 +58,7 @@ __global__ void __launch_bounds__(128, CURV ? 1 : OSBLI_YZ_MINB)
 sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
                 int chunk, const RkArgs rk) {
   static_assert(DIR == 1 || DIR == 2, "x has its own kernel");
-  __shared__ double stg[3][5][128];     // per-thread slots: R, dU of node q; Q of node q+4
+  __shared__ double stg[8][5][128];     // per-thread slots: R (0-2) and dU (3-5) of nodes n % 3, raw state (6-7) of nodes n & 1
   const Layout &Ly = P.L;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= Ly.n[0]) return;
@@ -110,16 +110,40 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
     if (m >= 3) rsq[m - 3] = rs;
     if (m == 3) rl = roe_side<CURV>(w[3], rs);   // node s0-1 = left node of the first interface
   }
-  // fused update on uniform grids: the next node's state is staged by cp.async too (measured: helps the
-  // fused z sweep, 0.98 -> 0.95 ms, costs the plain y sweep 0.84 -> 0.85 ms)
+  // Asynchronous staging, two iterations ahead (one iteration of flux arithmetic does not keep enough bytes in
+  // flight for HBM with 8 warps per SM): R (and dU) of node n travel by cp.async into the per-thread slot n % 3,
+  // issued while interface n-2 is computed; in the fused update on uniform grids the raw state of the node that
+  // enters the window is staged the same way (slot n & 1), elsewhere it is prefetched into registers.
   constexpr bool kAsyncQ = !CURV && RK != 0;
-  auto load_async = [&](int node) {
-    const long long o = line0 + (long long)node * st;
+  constexpr int kGroups = kAsyncQ ? 2 : 1;       // cp.async groups committed per iteration
+  auto issue_rd = [&](int node) {                // group 1: R, dU of `node` (empty outside [s0, s1))
+    if (node >= s0 && node < s1) {
+      const long long o = line0 + (long long)node * st;
+      if constexpr (ACCUM) {
 #pragma unroll
-    for (int c = 0; c < 5; ++c) cp_async8(&stg[2][c][threadIdx.x], Q + c * sv + o);
+        for (int c = 0; c < 5; ++c) cp_async8(&stg[node % 3][c][threadIdx.x], R + c * sv + o);
+      }
+      if constexpr (RK == 2) {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) cp_async8(&stg[3 + node % 3][c][threadIdx.x], rk.Qtmp + c * sv + o);
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  auto issue_q = [&](int node) {                 // group 2: raw state of `node` (needed up to node s1+2)
+    if (node <= s1 + 2) {
+      const long long o = line0 + (long long)node * st;
+#pragma unroll
+      for (int c = 0; c < 5; ++c) cp_async8(&stg[6 + (node & 1)][c][threadIdx.x], Q + c * sv + o);
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
   };
   double qn[5], Kn[3] = {0.0, 0.0, 0.0};
-  if constexpr (kAsyncQ) { load_async(s0 + 2); asm volatile("cp.async.commit_group;" ::: "memory"); }
+  // prologue = what iterations s0-3 and s0-2 would have issued
+  issue_rd(s0 - 1);
+  if constexpr (kAsyncQ) issue_q(s0 + 2);
+  issue_rd(s0);
+  if constexpr (kAsyncQ) issue_q(s0 + 3);
   else load(s0 + 2, qn, Kn);                     // prefetched raw state of the next node
 
   for (int q = s0 - 1; q < s1; ++q) {            // interface q+1/2, between nodes q and q+1
@@ -127,32 +151,16 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
     for (int m = 0; m < 5; ++m) w[m] = w[m + 1];
     rsq[0] = rsq[1]; rsq[1] = rsq[2];
     if constexpr (kAsyncQ) {
-      asm volatile("cp.async.wait_all;" ::: "memory");
+      asm volatile("cp.async.wait_group 2;" ::: "memory");      // node q+3 has landed (issued two iterations ago)
 #pragma unroll
-      for (int c = 0; c < 5; ++c) qn[c] = stg[2][c][threadIdx.x];
+      for (int c = 0; c < 5; ++c) qn[c] = stg[6 + ((q + 3) & 1)][c][threadIdx.x];
     }
     make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], w[5], rsq[2]);
     if constexpr (!kAsyncQ) {
       if (q + 1 < s1) load(q + 4, qn, Kn);       // node (q+1)+3, used by the next interface
     }
-    // R (and dU) of node q travel to per-thread shared-memory slots by cp.async while the flux is
-    // computed: no registers held, no wait until the values are needed
-    if (q >= s0) {
-      const long long o = line0 + (long long)q * st;
-      if constexpr (ACCUM) {
-#pragma unroll
-        for (int c = 0; c < 5; ++c) cp_async8(&stg[0][c][threadIdx.x], R + c * sv + o);
-      }
-      if constexpr (RK == 2) {
-#pragma unroll
-        for (int c = 0; c < 5; ++c) cp_async8(&stg[1][c][threadIdx.x], rk.Qtmp + c * sv + o);
-      }
-    }
-    asm volatile("cp.async.commit_group;" ::: "memory");       // group 1: R, dU of node q (may be empty)
-    if constexpr (kAsyncQ) {
-      if (q + 1 < s1) load_async(q + 4);                       // group 2: node (q+1)+3 for the next interface
-      asm volatile("cp.async.commit_group;" ::: "memory");
-    }
+    issue_rd(q + 2);
+    if constexpr (kAsyncQ) issue_q(q + 5);
     double rold[5] = {0, 0, 0, 0, 0};
     const RoeSide rr = roe_side<CURV>(w[3], rsq[0]);
     double f[5];
@@ -163,17 +171,18 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
       const long long o = line0 + (long long)q * st;
       double sc = inv_d;
       if constexpr (CURV) sc = 1.0 / __ldg(P.detJ + o);
-      if constexpr (kAsyncQ) asm volatile("cp.async.wait_group 1;" ::: "memory");   // group 1 done, group 2 may still fly
-      else asm volatile("cp.async.wait_all;" ::: "memory");
+      // R, dU of node q were issued two iterations ago: everything younger may still be in flight
+      if constexpr (kGroups == 2) asm volatile("cp.async.wait_group 4;" ::: "memory");
+      else asm volatile("cp.async.wait_group 2;" ::: "memory");
       if constexpr (ACCUM) {
 #pragma unroll
-        for (int c = 0; c < 5; ++c) rold[c] = stg[0][c][threadIdx.x];
+        for (int c = 0; c < 5; ++c) rold[c] = stg[q % 3][c][threadIdx.x];
       }
       if constexpr (RK != 0) {
         double dold[5] = {0, 0, 0, 0, 0};
         if constexpr (RK == 2) {
 #pragma unroll
-          for (int c = 0; c < 5; ++c) dold[c] = stg[1][c][threadIdx.x];
+          for (int c = 0; c < 5; ++c) dold[c] = stg[3 + q % 3][c][threadIdx.x];
         }
 #pragma unroll
         for (int c = 0; c < 5; ++c) {
