@@ -23,6 +23,8 @@ WENOZ5, TENO5, TENO6, WENOJS5, CENTRAL4, WENOZ3 = 0, 1, 2, 3, 4, 5
 VISC_NONE, VISC_CONST, VISC_SUTHERLAND = 0, 1, 2
 BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL = 0, 1, 2, 3
 PART_INVISCID, PART_VISCOUS = 1, 2
+AVG_ROE, AVG_SIMPLE = 0, 1
+RK3_WILLIAMSON, RK3_SSP = 0, 1
 
 _dp = C.POINTER(C.c_double)
 
@@ -45,6 +47,8 @@ class _Params(C.Structure):
         ("dirichlet", _dp),
         ("nthreads", C.c_int32),
         ("force", C.c_double * 3),
+        ("averaging", C.c_int32),
+        ("rk3_form", C.c_int32),
     ]
 
 
@@ -76,6 +80,10 @@ def lib():
         L.oracle_teno6_indicators.argtypes = [C.c_double] * 6 + [_dp]
         L.oracle_eigensystem.restype = None
         L.oracle_eigensystem.argtypes = [C.c_double, _dp, _dp, _dp, _dp, _dp, _dp]
+        L.oracle_eigensystem_avg.restype = None
+        L.oracle_eigensystem_avg.argtypes = [C.c_double, C.c_int32, _dp, _dp, _dp, _dp, _dp, _dp]
+        L.oracle_rk3ssp_update.restype = None
+        L.oracle_rk3ssp_update.argtypes = [C.c_int32, C.c_double, C.c_int64, _dp, _dp, _dp]
         L.oracle_d1.restype = C.c_double
         L.oracle_d1.argtypes = [_dp, C.c_int32, C.c_int32, C.c_int32, C.c_double]
         L.oracle_d2.restype = C.c_double
@@ -129,12 +137,12 @@ def teno6_indicators(a, b, c, d, e, f):
     return out
 
 
-def eigensystem(gamma, QL, QR, nhat):
+def eigensystem(gamma, QL, QR, nhat, averaging=AVG_ROE):
     QL = np.ascontiguousarray(QL, dtype=np.float64)
     QR = np.ascontiguousarray(QR, dtype=np.float64)
     nhat = np.ascontiguousarray(nhat, dtype=np.float64)
     L = np.zeros((5, 5)); R = np.zeros((5, 5)); roe = np.zeros(5)
-    lib().oracle_eigensystem(gamma, _ptr(QL), _ptr(QR), _ptr(nhat), _ptr(L), _ptr(R), _ptr(roe))
+    lib().oracle_eigensystem_avg(gamma, int(averaging), _ptr(QL), _ptr(QR), _ptr(nhat), _ptr(L), _ptr(R), _ptr(roe))
     return L, R, roe
 
 
@@ -156,6 +164,11 @@ def d2(f, i, periodic, delta, pad=0):
 def rk4_update(s, dt, U, dU, R):
     """One sub-stage (s = 0..4) of the five-stage 4th-order scheme on flat arrays, in place."""
     lib().oracle_rk4_update(int(s), float(dt), U.size, _ptr(U), _ptr(dU), _ptr(R))
+
+
+def rk3ssp_update(s, dt, U, dU, R):
+    """One sub-stage (s = 0..2) of the SSP 3rd-order scheme on flat arrays, in place."""
+    lib().oracle_rk3ssp_update(int(s), float(dt), U.size, _ptr(U), _ptr(dU), _ptr(R))
 
 
 def rk3_update(s, dt, U, dU, R):
@@ -196,7 +209,7 @@ class Oracle:
     def __init__(self, *, n, delta=(1.0, 1.0, 1.0), metrics=None, gamma=1.4, Re=1.0, Pr=1.0, Minf=1.0,
                  scheme=WENOZ5, teno_ct=1e-6, eps=1e-16, visc=VISC_NONE, suth_ratio=110.4 / 288.0,
                  bc=((0, 0), (0, 0), (0, 0)), wall_T=((0, 0), (0, 0), (0, 0)), dirichlet=None,
-                 nthreads=None, force=(0.0, 0.0, 0.0)):
+                 nthreads=None, force=(0.0, 0.0, 0.0), averaging=AVG_ROE, rk3_form=RK3_WILLIAMSON):
         self.n = tuple(int(v) for v in n)
         self.h = tuple(3 if v > 1 else 0 for v in self.n)
         self.N = tuple(v + 2 * h for v, h in zip(self.n, self.h))
@@ -237,6 +250,8 @@ class Oracle:
             p.dirichlet = _ptr(a)
         p.nthreads = self.nthreads
         p.force[:] = [float(v) for v in force]
+        p.averaging = int(averaging)
+        p.rk3_form = int(rk3_form)
         self.p = p
 
     def _field(self, a):

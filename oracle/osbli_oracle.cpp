@@ -212,22 +212,36 @@ double reconstruct6(double a, double b, double c, double d, double e, double f,
 }
 
 /* ---------------------------------------------------------- Roe-averaged eigensystem ---- */
-/* PAPER.md:104-105, steps 2(a)-(b).  Roe average: u_j and H with sqrt(rho) weights, a~ from
- * H~ (Q11).  Eigenvectors for a general unit normal n without tangent vectors
+/* PAPER.md:104-105, steps 2(a)-(b): "Compute the average U_{i+1/2} state with either simple or Roe
+ * averaging."  Roe average (averaging == ORACLE_AVG_ROE): u_j and H with sqrt(rho) weights, a~ from
+ * H~ (Q11).  Simple average (ORACLE_AVG_SIMPLE, Q38): the arithmetic mean of the
+ * two conservative states, U_{i+1/2} = (U_i + U_{i+1})/2, and u_j, H, a of THAT state.
+ * Eigenvectors for a general unit normal n without tangent vectors
  * (Q12); fields ordered 0,1,2 (speed theta), 3 (theta+a), 4 (theta-a). */
-void eigensystem(double gamma, const double *QL, const double *QR, const double *n,
+void eigensystem(double gamma, int averaging, const double *QL, const double *QR, const double *n,
                  double *L, double *R, double *roe) {
-  const double rL = QL[0], rR = QR[0];
-  const double uL = QL[1] / rL, vL = QL[2] / rL, wL = QL[3] / rL;
-  const double uR = QR[1] / rR, vR = QR[2] / rR, wR = QR[3] / rR;
-  const double pL = (gamma - 1.0) * (QL[4] - 0.5 * rL * (uL * uL + vL * vL + wL * wL));
-  const double pR = (gamma - 1.0) * (QR[4] - 0.5 * rR * (uR * uR + vR * vR + wR * wR));
-  const double HL = (QL[4] + pL) / rL, HR = (QR[4] + pR) / rR;
-  const double sl = std::sqrt(rL), sr = std::sqrt(rR);
-  const double u = (sl * uL + sr * uR) / (sl + sr);
-  const double v = (sl * vL + sr * vR) / (sl + sr);
-  const double w = (sl * wL + sr * wR) / (sl + sr);
-  const double H = (sl * HL + sr * HR) / (sl + sr);
+  double u, v, w, H;
+  if (averaging == ORACLE_AVG_SIMPLE) {
+    double qm[5];
+    for (int c = 0; c < 5; ++c) qm[c] = 0.5 * (QL[c] + QR[c]);
+    u = qm[1] / qm[0];
+    v = qm[2] / qm[0];
+    w = qm[3] / qm[0];
+    const double pm = (gamma - 1.0) * (qm[4] - 0.5 * qm[0] * (u * u + v * v + w * w));
+    H = (qm[4] + pm) / qm[0];
+  } else {
+    const double rL = QL[0], rR = QR[0];
+    const double uL = QL[1] / rL, vL = QL[2] / rL, wL = QL[3] / rL;
+    const double uR = QR[1] / rR, vR = QR[2] / rR, wR = QR[3] / rR;
+    const double pL = (gamma - 1.0) * (QL[4] - 0.5 * rL * (uL * uL + vL * vL + wL * wL));
+    const double pR = (gamma - 1.0) * (QR[4] - 0.5 * rR * (uR * uR + vR * vR + wR * wR));
+    const double HL = (QL[4] + pL) / rL, HR = (QR[4] + pR) / rR;
+    const double sl = std::sqrt(rL), sr = std::sqrt(rR);
+    u = (sl * uL + sr * uR) / (sl + sr);
+    v = (sl * vL + sr * vR) / (sl + sr);
+    w = (sl * wL + sr * wR) / (sl + sr);
+    H = (sl * HL + sr * HR) / (sl + sr);
+  }
   const double q2 = u * u + v * v + w * w;
   const double a = std::sqrt((gamma - 1.0) * (H - 0.5 * q2));
   const double nx = n[0], ny = n[1], nz = n[2];
@@ -306,7 +320,7 @@ void interface_flux(const oracle_params *p, const Grid &g, const double *Q, int 
     nhat[0] = kx / kn; nhat[1] = ky / kn; nhat[2] = kz / kn;
   }
   double L[25], R[25];
-  eigensystem(p->gamma, U[2], U[3], nhat, L, R, nullptr);
+  eigensystem(p->gamma, p->averaging, U[2], U[3], nhat, L, R, nullptr);
 
   for (int c = 0; c < 5; ++c) fhat[c] = 0.0;
   double mmin = std::numeric_limits<double>::infinity();
@@ -648,6 +662,8 @@ int validate(const oracle_params *p) {
     if ((p->bc[d][0] == ORACLE_BC_PERIODIC) != (p->bc[d][1] == ORACLE_BC_PERIODIC)) return 1;
   }
   if (p->nthreads < 1) return 1;
+  if (p->averaging != ORACLE_AVG_ROE && p->averaging != ORACLE_AVG_SIMPLE) return 1;
+  if (p->rk3_form != ORACLE_RK3_WILLIAMSON && p->rk3_form != ORACLE_RK3_SSP) return 1;
   if (p->scheme == ORACLE_CENTRAL4 && p->curvilinear) return 1;   /* central convective terms: uniform grids only */
   return 0;
 }
@@ -855,7 +871,11 @@ void oracle_teno6_indicators(double a, double b, double c, double d, double e, d
 
 void oracle_eigensystem(double gamma, const double *QL, const double *QR, const double *nhat,
                         double *L, double *R, double *roe) {
-  eigensystem(gamma, QL, QR, nhat, L, R, roe);
+  eigensystem(gamma, ORACLE_AVG_ROE, QL, QR, nhat, L, R, roe);
+}
+void oracle_eigensystem_avg(double gamma, int32_t averaging, const double *QL, const double *QR,
+                            const double *nhat, double *L, double *R, double *roe) {
+  eigensystem(gamma, averaging, QL, QR, nhat, L, R, roe);
 }
 
 double oracle_d1(const double *f, int32_t n, int32_t i, int32_t per, double delta) {
@@ -952,6 +972,21 @@ void oracle_rk3_update(int32_t s, double dt, int64_t count, double *U, double *d
   }
 }
 
+/* "plus a 3rd order strong-stability-preserving (SSP) version to improve stability for flows containing
+ * discontinuities ... [44] for the SSP version of the 3rd order scheme" (used by the
+ * problem script at PAPER.md:343).  Same form eq. (36)-(38); the coefficients are not printed: the three-stage
+ * 2N-storage TVD scheme of Gottlieb & Shu, as published to six digits in B_1 (Q39).  A_3 = 0: the
+ * last stage is a plain Euler increment from U^(2). */
+void oracle_rk3ssp_update(int32_t s, double dt, int64_t count, double *U, double *dU, const double *R) {
+  const double A[3] = {0.0, -2.915493957701923, 0.0};
+  const double B[3] = {0.924574, 0.287713063186749, 0.626538109512740};
+  for (int64_t o = 0; o < count; ++o) {
+    const double du = (A[s] == 0.0 ? 0.0 : A[s] * dU[o]) + dt * R[o];          /* eq. (36) */
+    dU[o] = du;
+    U[o] = U[o] + B[s] * du;                                                    /* eq. (37) */
+  }
+}
+
 /* The 4th-order member of the same low-storage family eq. (36)-(38): "The 3rd and 4th order schemes have
  * three and five sub-stages per iteration respectively. The coefficients A_i and B_i are taken from [23]"
  * (PAPER.md:242): the five-stage 2N-storage scheme of Carpenter & Kennedy (Q35). */
@@ -998,7 +1033,8 @@ int32_t oracle_rk3_step(const oracle_params *p, double *Q, double *dU, double *R
       for (int j = 0; j < g.n[1]; ++j)
         for (int c = 0; c < 5; ++c) {
           const long o = c * g.total + g.idx(0, j, k);
-          oracle_rk3_update(s, dt, g.n[0], Q + o, dU + o, R + o);
+          if (p->rk3_form == ORACLE_RK3_SSP) oracle_rk3ssp_update(s, dt, g.n[0], Q + o, dU + o, R + o);
+          else                               oracle_rk3_update(s, dt, g.n[0], Q + o, dU + o, R + o);
         }
   }
   for (int d = 0; d < 3; ++d) bc_direction(p, g, Q, d);

@@ -37,6 +37,8 @@ enum { ORACLE_VISC_NONE = 0, ORACLE_VISC_CONST = 1, ORACLE_VISC_SUTHERLAND = 2 }
 enum { ORACLE_BC_PERIODIC = 0, ORACLE_BC_EXTRAP0 = 1, ORACLE_BC_DIRICHLET = 2, ORACLE_BC_WALL_ISOTHERMAL = 3,
        ORACLE_BC_WALL_ADIABATIC = 4 };
 enum { ORACLE_PART_INVISCID = 1, ORACLE_PART_VISCOUS = 2 };
+enum { ORACLE_AVG_ROE = 0, ORACLE_AVG_SIMPLE = 1 };            /* PAPER.md:104 step 2(a)                    */
+enum { ORACLE_RK3_WILLIAMSON = 0, ORACLE_RK3_SSP = 1 };        /* PAPER.md:232, 242 (refs [23], [44])       */
 
 typedef struct {
   int32_t n[3];           /* interior points nx, ny, nz; n_d == 1 => direction inactive             */
@@ -57,6 +59,8 @@ typedef struct {
   int32_t nthreads;       /* OpenMP threads for the outer line loops (>= 1)                         */
   double  force[3];       /* constant body force per unit volume (channel case):  */
                           /* R_{rho u_i} += f_i, R_{rho E} += u_i f_i (Q34)               */
+  int32_t averaging;      /* ORACLE_AVG_*: interface state of step 2(a) (Q11, Q38)        */
+  int32_t rk3_form;       /* ORACLE_RK3_*: coefficients used by oracle_rk3_step (Q15, Q39) */
 } oracle_params;
 
 /* ---- building blocks, exposed so that the pins can reach them one by one ---------------- */
@@ -81,6 +85,10 @@ void oracle_teno6_indicators(double a, double b, double c, double d, double e, d
  * eigenvectors), R (columns = right eigenvectors), and the Roe state (u,v,w,H,a). */
 void oracle_eigensystem(double gamma, const double *QL, const double *QR, const double *nhat,
                         double *L, double *R, double *roe);
+
+/* Same with the averaging of step 2(a) selectable (ORACLE_AVG_*; Q38). */
+void oracle_eigensystem_avg(double gamma, int32_t averaging, const double *QL, const double *QR,
+                            const double *nhat, double *L, double *R, double *roe);
 
 /* 4th-order central first / second difference of a 1-D array f[0..n-1] at node i
  * (eq. 28 (sign corrected), 29, 30-35).  periodic != 0: f must carry 2
@@ -124,8 +132,12 @@ int32_t oracle_metrics(const oracle_params *p, const double *coords,
  * (eq. 36-37; s = 0,1,2).  oracle_rk3_step applies exactly this per x-line. */
 void oracle_rk3_update(int32_t s, double dt, int64_t count, double *U, double *dU, const double *R);
 
+/* The SSP member of the 3rd-order family (coefficients: DESIGN.md Q39). */
+void oracle_rk3ssp_update(int32_t s, double dt, int64_t count, double *U, double *dU, const double *R);
+
 /* One low-storage RK3 step (eq. 36-38): for s in 0..2 { bc(Q); R = rhs(Q);
- * dU = A_s dU + dt R; Q += B_s dU }; bc(Q).  dU and R are caller-provided scratch states. */
+ * dU = A_s dU + dt R; Q += B_s dU }; bc(Q).  dU and R are caller-provided scratch states.
+ * p->rk3_form selects the coefficient set (Williamson [23] or SSP [44]). */
 int32_t oracle_rk3_step(const oracle_params *p, double *Q, double *dU, double *R, double dt);
 
 /* Five-stage 4th-order member of the same family (Q35). */

@@ -23,6 +23,8 @@ import numpy as np
 WENOZ5, TENO5, TENO6, WENOJS5, CENTRAL4, WENOZ3 = 0, 1, 2, 3, 4, 5
 VISC_NONE, VISC_CONST, VISC_SUTHERLAND = 0, 1, 2
 BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL, BC_WALL_ADIABATIC = 0, 1, 2, 3, 4
+AVG_ROE, AVG_SIMPLE = 0, 1
+RK3_WILLIAMSON, RK3_SSP = 0, 1
 
 
 @dataclass
@@ -47,6 +49,8 @@ class Case:
     wall_T: tuple = ((0.0, 0.0), (0.0, 0.0), (0.0, 0.0))
     dirichlet: Optional[np.ndarray] = None     # [5, NZ, NY, NX] frozen boundary state
     force: tuple = (0.0, 0.0, 0.0)             # constant body force per unit volume
+    averaging: int = AVG_ROE                   # interface state of step 2(a)
+    rk3_form: int = RK3_WILLIAMSON             # coefficient set of the 3-stage scheme
     extra: dict = field(default_factory=dict)  # analytic solutions etc. for the pins
 
     @property
@@ -66,7 +70,7 @@ class Case:
         return dict(n=self.n, delta=self.delta, gamma=self.gamma, Re=self.Re, Pr=self.Pr, Minf=self.Minf,
                     scheme=self.scheme, teno_ct=self.teno_ct, eps=self.eps, visc=self.visc,
                     suth_ratio=self.suth_ratio, bc=self.bc, wall_T=self.wall_T, dirichlet=self.dirichlet,
-                    force=self.force)
+                    force=self.force, averaging=self.averaging, rk3_form=self.rk3_form)
 
 
 # ------------------------------------------------------------------------------ helpers ----
