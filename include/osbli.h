@@ -53,6 +53,10 @@ enum { OSBLI_VISC_NONE = 0 /* Euler */, OSBLI_VISC_CONST = 1 /* mu = 1 */,
        OSBLI_VISC_SUTHERLAND = 2 /* PAPER.md:59-63, 317-318 */ };
 enum { OSBLI_BC_PERIODIC = 0, OSBLI_BC_EXTRAP0 = 1, OSBLI_BC_DIRICHLET = 2,
        OSBLI_BC_WALL_ISOTHERMAL = 3, OSBLI_BC_WALL_ADIABATIC = 4 };             /* PAPER.md:355-387, 586 */
+enum { OSBLI_AVG_ROE = 0 /* sqrt(rho)-weighted u_j, H */,
+       OSBLI_AVG_SIMPLE = 1 /* U_{i+1/2} = (U_i + U_{i+1})/2 */ };               /* PAPER.md:104 step 2(a) */
+enum { OSBLI_RK3_WILLIAMSON = 0 /* coefficients of ref. [23] */,
+       OSBLI_RK3_SSP = 1 /* strong-stability-preserving set of ref. [44] */ };   /* PAPER.md:232, 242, 343 */
 
 /* Curvilinear metric fields (PAPER.md:228), DEVICE pointers, each one scalar field in the
  * padded layout with halos filled.  Unit computational spacing in every direction. */
@@ -85,6 +89,9 @@ typedef struct {
                               boundary values, required iff some bc == OSBLI_BC_DIRICHLET        */
   double  force[3];        /* constant body force per unit volume (laminar channel):
                               dQ/dt gains f_i in the momentum and u_i f_i in the energy equation  */
+  int32_t averaging;       /* OSBLI_AVG_*: interface state whose eigenvectors diagonalise the fluxes,
+                              PAPER.md:104 "either simple or Roe averaging"                        */
+  int32_t rk3_form;        /* OSBLI_RK3_*: coefficient set A_i, B_i used by osbli_rk3_step          */
 } osbli_params;
 
 typedef struct {
@@ -127,6 +134,7 @@ int osbli_rhs(osbli_handle h, const double *d_Q, double *d_R, void *cuda_stream)
 /* One low-storage RK3 step, eq. (36)-(38): for s in 0..2 { bc(Q); R = rhs(Q);
  * Qtmp = A_s Qtmp + dt R; Q += B_s Qtmp } then bc(Q).  d_Qtmp is the dU accumulator of eq. (36);
  * it is overwritten (A_0 = 0) and need not be initialised.  R lives in the workspace.
+ * A_i, B_i: params.rk3_form (Williamson's 2N-storage scheme, or the SSP set whose A_3 is 0 as well).
  * With two or more active directions the update is done by the last sweep kernel of each stage
  * (no separate pass over R), which cannot update in place: the state moves d_Q -> Q2 -> Q3 ->
  * d_Q through two workspace states; the result is in d_Q with its halos filled.  The viscous

@@ -53,6 +53,8 @@ int validate(const osbli_params *p) {
   if (p->scheme < OSBLI_SCHEME_WENOZ5 || p->scheme > OSBLI_SCHEME_WENOZ3) return OSBLI_EINVAL;
   if (p->scheme == OSBLI_SCHEME_CENTRAL4 && p->metrics) return OSBLI_EUNSUPPORTED;   // central convective terms: uniform grids
   if (p->visc < OSBLI_VISC_NONE || p->visc > OSBLI_VISC_SUTHERLAND) return OSBLI_EINVAL;
+  if (p->averaging != OSBLI_AVG_ROE && p->averaging != OSBLI_AVG_SIMPLE) return OSBLI_EINVAL;
+  if (p->rk3_form != OSBLI_RK3_WILLIAMSON && p->rk3_form != OSBLI_RK3_SSP) return OSBLI_EINVAL;
   if (!(p->gamma > 1.0)) return OSBLI_EINVAL;
   if (!(p->eps >= 1e-18) || !(p->teno_ct > 0.0)) return OSBLI_EINVAL;
   if (p->visc != OSBLI_VISC_NONE && (!(p->Re > 0.0) || !(p->Pr > 0.0) || !(p->Minf > 0.0))) return OSBLI_EINVAL;
@@ -162,8 +164,8 @@ int do_step(osbli_ctx *h, int nstages, double *Q, double *Qtmp, double dt, cudaS
       if (s == 0 || !wrap)
         if (int rc = do_bc(h, src, st)) return rc;
       RkArgs rk;
-      rk_coefficients(nstages, s, &rk.A, &rk.B);
-      rk.dt = dt; rk.Qtmp = Qtmp; rk.Qout = dst; rk.first = (s == 0); rk.wrap = wrap ? 1 : 0;
+      rk_coefficients(nstages, h->P.rk3_form, s, &rk.A, &rk.B);
+      rk.dt = dt; rk.Qtmp = Qtmp; rk.Qout = dst; rk.first = (rk.A == 0.0); rk.wrap = wrap ? 1 : 0;   // A_s = 0: dU is not read
       if (int rc = do_rhs(h, src, h->R, &rk, st)) return rc;
     } else {
       if (int rc = do_bc(h, Q, st)) return rc;
@@ -239,6 +241,8 @@ int osbli_init(const osbli_params *p, void *d_workspace, size_t workspace_bytes,
   P.dirichlet = p->dirichlet;
   for (int a = 0; a < 3; ++a) P.force[a] = p->force[a];
   P.has_force = (p->force[0] != 0.0 || p->force[1] != 0.0 || p->force[2] != 0.0) ? 1 : 0;
+  P.averaging = p->averaging;
+  P.rk3_form = p->rk3_form;
   if (p->metrics) {
     for (int k = 0; k < 3; ++k) {
       for (int j = 0; j < 3; ++j) P.D[k][j] = p->metrics->D[k][j];

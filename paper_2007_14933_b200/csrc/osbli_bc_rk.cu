@@ -165,7 +165,12 @@ rk_update_kernel(const __grid_constant__ DevParams P, double A, double B, double
 
 // Coefficients of eq. (36)-(37) "from [23]": nstages = 3 -> Williamson's 2N-storage RK3
 // (Q15); nstages = 5 -> Carpenter & Kennedy's five-stage 4th-order 2N-storage scheme (Q35).
-void rk_coefficients(int nstages, int stage, double *A, double *B) {
+// form = 1 (nstages = 3 only): the strong-stability-preserving 2N-storage set of ref. [44] (
+// DESIGN.md Q39), as published (B_1 to six digits); its A_3 is 0, so the last stage does not read dU.
+void rk_coefficients(int nstages, int form, int stage, double *A, double *B) {
+  static const double as3[3] = {0.0, -2.915493957701923, 0.0};
+  static const double bs3[3] = {0.924574, 0.287713063186749, 0.626538109512740};
+  if (nstages == 3 && form == 1) { *A = as3[stage]; *B = bs3[stage]; return; }
   static const double a3[3] = {0.0, -5.0 / 9.0, -153.0 / 128.0};
   static const double b3[3] = {1.0 / 3.0, 15.0 / 16.0, 8.0 / 15.0};
   static const double a5[5] = {0.0, -567301805773.0 / 1357537059087.0, -2404267990393.0 / 2016746695238.0,
@@ -180,11 +185,11 @@ void rk_coefficients(int nstages, int stage, double *A, double *B) {
 cudaError_t launch_rk_update(const DevParams &P, int nstages, int stage, double dt, double *Q, double *Qtmp,
                              const double *R, cudaStream_t st) {
   double A, B;
-  rk_coefficients(nstages, stage, &A, &B);
+  rk_coefficients(nstages, P.rk3_form, stage, &A, &B);
   const Layout &L = P.L;
   const int pairs = (L.n[0] + 1) / 2;
   dim3 grid((pairs + 127) / 128, L.n[1], L.n[2]);
-  if (stage == 0) rk_update_kernel<true><<<grid, 128, 0, st>>>(P, A, B, dt, Q, Qtmp, R);
+  if (A == 0.0) rk_update_kernel<true><<<grid, 128, 0, st>>>(P, A, B, dt, Q, Qtmp, R);
   else rk_update_kernel<false><<<grid, 128, 0, st>>>(P, A, B, dt, Q, Qtmp, R);
   return cudaGetLastError();
 }

@@ -9,7 +9,7 @@ namespace osbli {
 // wrap != 0 (all active directions periodic): the periodic images of the boundary-near nodes are
 // written into the halos of Qout as well, which replaces the halo fill of the next stage.
 struct RkArgs { double A, B, dt; double *Qtmp, *Qout; int first, wrap; };
-void rk_coefficients(int nstages, int stage, double *A, double *B);   // nstages = 3 (RK3) or 5 (RK4)
+void rk_coefficients(int nstages, int form, int stage, double *A, double *B);   // nstages = 3 (RK3; form = OSBLI_RK3_*) or 5 (RK4)
 
 // R (-)= flux difference of the characteristic reconstruction along `dir` (osbli_sweep.cu).
 // rk != nullptr (dir 1 or 2, accumulate = 1 only): R is read but not written, the stage update is done instead.

@@ -108,7 +108,7 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
     double rs;
     make_point<DIR, CURV>(P, q[0], q[1], q[2], q[3], q[4], K[0], K[1], K[2], w[m], rs);
     if (m >= 3) rsq[m - 3] = rs;
-    if (m == 3) rl = roe_side<CURV>(w[3], rs);   // node s0-1 = left node of the first interface
+    if (m == 3) rl = roe_side<CURV>(P, w[3], rs);   // node s0-1 = left node of the first interface
   }
   // Asynchronous staging, two iterations ahead (one iteration of flux arithmetic does not keep enough bytes in
   // flight for HBM with 8 warps per SM): R (and dU) of node n travel by cp.async into the per-thread slot n % 3,
@@ -162,7 +162,7 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
     issue_rd(q + 2);
     if constexpr (kAsyncQ) issue_q(q + 5);
     double rold[5] = {0, 0, 0, 0, 0};
-    const RoeSide rr = roe_side<CURV>(w[3], rsq[0]);
+    const RoeSide rr = roe_side<CURV>(P, w[3], rsq[0]);
     double f[5];
     if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, rl, rr, rp, f);
     else interface_flux<DIR, SCHEME>(P, w, rl, rr, rp, f);
@@ -329,9 +329,9 @@ sweep_x_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q
       make_point<0, CURV>(P, r, mx, my, mz, E, kx, ky, kz, w[5], rsq[2]);
     }
     const int q = node - 3;                                      // interface q+1/2 is now computable
-    if (q == s0 - 2) rl = roe_side<CURV>(w[3], rsq[0]);         // slot 3 holds node s0-1
+    if (q == s0 - 2) rl = roe_side<CURV>(P, w[3], rsq[0]);         // slot 3 holds node s0-1
     if (q < s0 - 1) continue;
-    const RoeSide rr = roe_side<CURV>(w[3], rsq[0]);
+    const RoeSide rr = roe_side<CURV>(P, w[3], rsq[0]);
     double f[5];
     if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, rl, rr, rp, f);
     else interface_flux<0, SCHEME>(P, w, rl, rr, rp, f);

@@ -28,6 +28,8 @@ OK, EINVAL, EUNSUPPORTED, ECUDA, EWORKSPACE = 0, 1, 2, 3, 4
 SCHEME_WENOZ5, SCHEME_TENO5, SCHEME_TENO6, SCHEME_WENOJS5, SCHEME_CENTRAL4, SCHEME_WENOZ3 = 0, 1, 2, 3, 4, 5
 VISC_NONE, VISC_CONST, VISC_SUTHERLAND = 0, 1, 2
 BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL, BC_WALL_ADIABATIC = 0, 1, 2, 3, 4
+AVG_ROE, AVG_SIMPLE = 0, 1
+RK3_WILLIAMSON, RK3_SSP = 0, 1
 
 _dp = C.c_void_p   # device / host addresses travel as plain integers
 
@@ -50,6 +52,8 @@ class Params(C.Structure):
         ("wall_T", (C.c_double * 2) * 3),
         ("dirichlet", _dp),
         ("force", C.c_double * 3),
+        ("averaging", C.c_int32),
+        ("rk3_form", C.c_int32),
     ]
 
 
@@ -180,7 +184,7 @@ def osbli_destroy(handle):
 def make_params(*, n, delta=(1.0, 1.0, 1.0), gamma=1.4, Re=1.0, Pr=1.0, Minf=1.0, scheme=SCHEME_WENOZ5,
                 teno_ct=1e-6, eps=1e-16, visc=VISC_NONE, suth_ratio=110.4 / 288.0,
                 bc=((0, 0), (0, 0), (0, 0)), wall_T=((0.0, 0.0), (0.0, 0.0), (0.0, 0.0)), force=(0.0, 0.0, 0.0),
-                **_ignored) -> Params:
+                averaging=AVG_ROE, rk3_form=RK3_WILLIAMSON) -> Params:
     p = Params()
     p.nx, p.ny, p.nz = (int(v) for v in n)
     p.dx, p.dy, p.dz = (float(v) for v in delta)
@@ -192,6 +196,7 @@ def make_params(*, n, delta=(1.0, 1.0, 1.0), gamma=1.4, Re=1.0, Pr=1.0, Minf=1.0
             p.bc[d][s] = int(bc[d][s])
             p.wall_T[d][s] = float(wall_T[d][s])
     p.force[:] = [float(v) for v in force]
+    p.averaging, p.rk3_form = int(averaging), int(rk3_form)
     return p
 
 

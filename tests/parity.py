@@ -15,8 +15,10 @@ Tolerance on a single residual evaluation (per variable c, absolute):
   characteristic fluxes of size (|u|+a) rho that cancel only to rounding; + (|u|+a) p for energy).  At low Mach
   number Phi_c/Delta is ~1e5-1e6 times ||R_c||, so 1e-11 relative is below one rounding error of
   the terms being subtracted: the oracle compiled with FMA contraction (same source, same
-  operation order) already differs from itself by 3.7e-11 on the 64^3 TGV, i.e. ~3 of these units
-  (tests/test_tolerance_floor.py pins that on the CPU).  K_ULP = 32 such units are allowed.
+  operation order) already differs from itself by 3.7e-11 on the 64^3 TGV, i.e. ~3 of these units,
+  and flipping the last bit of the oracle's INPUT moves its own residual by 2-6 units in every
+  variable of every case, the spanwise momentum of the slab included (tests/test_tolerance_floor.py
+  pins both on the CPU).  K_ULP = 16 such units are allowed (worst observed on the GPU: 11.3).
 On the well-conditioned cases (Sod, Mach-2 boxes) the first term is the larger one and the stated
 1e-11 applies unchanged.
 """
@@ -30,7 +32,7 @@ import numpy as np
 
 from oracle import oracle as O
 
-K_ULP = 32.0
+K_ULP = 16.0
 U = 2.0 ** -53
 REL = 1e-11
 
@@ -95,8 +97,10 @@ def l1_rel(a, b):
     return out
 
 
-def flux_scale(case, Qi, metrics=None, points=None):
-    """max over (the given) interior nodes of Phi_c * sum_d |grad xi_d|; Qi = interior state [5,nz,ny,nx]."""
+def flux_scale(case, Qi, metrics=None, points=None, momentum_rho_term=True):
+    """max over (the given) interior nodes of Phi_c * sum_d |grad xi_d|; Qi = interior state [5,nz,ny,nx].
+    momentum_rho_term=False gives the first version of the model (momentum floor without (|u|+a) rho), kept only
+    so that tests/test_tolerance_floor.py can show what it misses."""
     g = case.gamma
     rho = Qi[0]
     u, v, w = Qi[1] / rho, Qi[2] / rho, Qi[3] / rho
@@ -115,8 +119,9 @@ def flux_scale(case, Qi, metrics=None, points=None):
     # momentum: the eigenvectors of DESIGN.md Q12 carry entries of unit size
     # (n_z, -n_y, ...) in the momentum rows of the three theta-fields, so every momentum component
     # receives characteristic fluxes of size (|u|+a) rho whatever its own magnitude is
+    mr = rho if momentum_rho_term else 0.0
     phi = [speed * np.abs(Qi[0]),
-           speed * (np.abs(Qi[1]) + rho) + p, speed * (np.abs(Qi[2]) + rho) + p, speed * (np.abs(Qi[3]) + rho) + p,
+           speed * (np.abs(Qi[1]) + mr) + p, speed * (np.abs(Qi[2]) + mr) + p, speed * (np.abs(Qi[3]) + mr) + p,
            speed * (np.abs(Qi[4]) + p)]
     return np.array([float((f * geo).max()) for f in phi])
 

@@ -357,6 +357,13 @@ def test_full_size_tgv256_config3_sampled():
     sampled_full_size("tgv256_sampled", 256, 3000, presteps=2)
 
 
+def test_full_size_tgv256_config3_state_3_steps():
+    """Whole 256^3 state (every node, halos included) against the oracle after 3 steps: complements the
+    configured-length test below, which compares a node sample."""
+    case = W.tgv(256)
+    run_steps_case("tgv256_3", case, 3, 1e-9, parity.q28)
+
+
 def test_full_size_tgv512_config5_sampled():
     torch = _torch()
     free, total = torch.cuda.mem_get_info()
@@ -366,26 +373,84 @@ def test_full_size_tgv512_config5_sampled():
     sampled_full_size("tgv512_sampled", 512, 1500, presteps=1)
 
 
-def _full_length():
-    import os
-    return os.environ.get("OSBLI_FULL_LENGTH", "0") == "1"
+# ------------------------------ configured-length parity against stored oracle samples ----
+def run_golden_config(config):
+    """BASELINE.json configs 3, 4, 5 for their CONFIGURED step counts (200 / 500 / 50) on the GPU, compared on the
+    strided node sample that oracle/make_golden.py stored from the oracle's own full-length run
+    (tests/golden/config{N}_oracle_samples.npz; hours of CPU time, done once).  The file must carry the hash of
+    the oracle sources as they are now, and the sampled initial state must be the one this run starts from.
+    north_star: max relative difference <= 1e-9 (smooth cases), L1 <= 1e-9 (shocked case), Q28 norms
+    with the oracle's full-field max-norms as denominators."""
+    import json
+    from oracle import make_golden as G
+    torch = _torch()
+    path = G.golden_path(config)
+    assert path.exists(), f"{path} missing: run `python oracle/make_golden.py --config {config}`"
+    z = np.load(path)
+    meta = json.loads(str(z["meta"]))
+    assert not meta["partial"], "stored oracle run stopped before the configured step count"
+    assert meta["oracle_sha256"] == G.oracle_source_hash(), (
+        f"{path.name} was written by a different oracle source: rerun `python oracle/make_golden.py --config {config}`")
+    make, stride, checkpoints = G.CONFIGS[config]
+    case = make()
+    assert meta["nsteps"] == case.nsteps == checkpoints[-1] and meta["dt"] == case.dt and tuple(meta["n"]) == tuple(case.n)
+    assert G.sample_hash(G.sample_of(case, case.Q0, stride)) == meta["q0_sample_sha256"], "input generator changed"
+    metrics = parity.metrics_for(case)
+    sol = parity.make_solver(case, metrics)
+    Q = sol.to_padded(case.Q0)
+    Qtmp = sol.empty_state()
+    lay, h, n = sol.layout, case.halo, case.n
+    norm = "l1" if config == 4 else "max"
+    step, worst = 0, None
+    for cp in checkpoints:
+        while step < cp:
+            sol.rk3_step(Q, Qtmp, case.dt)
+            step += 1
+        torch.cuda.synchronize()
+        smp = Q[:, h[2]:h[2] + n[2]:stride[2], h[1]:h[1] + n[1]:stride[1],
+                lay.x_offset:lay.x_offset + n[0]:stride[0]].cpu().numpy()
+        ref = z[f"state_{cp}"]
+        assert smp.shape == ref.shape and np.isfinite(smp).all()
+        den = z[f"maxnorm_{cp}"].copy()
+        den[den < 1e-12 * den.max()] = den.max()
+        d = np.abs(smp - ref).reshape(5, -1)
+        err = (d.mean(axis=1) if norm == "l1" else d.max(axis=1)) / den
+        parity.report(test=f"config{config}_golden", kind="state_sampled", nsteps=cp, norm=norm, err=err.tolist(),
+                      err_max_norm=(d.max(axis=1) / den).tolist(), tol=1e-9, nsamples=int(d.shape[1]))
+        worst = err
+        assert err.max() <= 1e-9, (config, cp, err)
+    assert step == case.nsteps
+    sol.close()
+    return worst
 
 
-def test_full_size_tgv256_config3_state():
-    """BASELINE.json config 3 at full size in the launch configuration bench.py times: the whole state
-    against the oracle after 3 steps (default; ~25 s of oracle time on 16 cores) or after all 200
-    (OSBLI_FULL_LENGTH=1, ~30 min), max relative difference <= 1e-9."""
-    case = W.tgv(256)
-    nsteps = case.nsteps if _full_length() else 3
-    run_steps_case(f"tgv256_{nsteps}", case, nsteps, 1e-9, parity.q28)
+def test_config3_tgv256_full_length():
+    """200 RK3 steps at 256^3 (the launch configuration bench.py times), 50 653 sampled nodes, max-norm <= 1e-9."""
+    run_golden_config(3)
 
 
-def test_full_size_tgv512_config5_state():
-    """BASELINE.json config 5: the 50 steps at 512^3 need ~1 h of oracle time; only with OSBLI_FULL_LENGTH=1
-    (OSBLI_C5_STEPS overrides the step count).  The default suite covers this size by sampled nodes above."""
-    import os
-    if not _full_length():
-        pytest.skip("set OSBLI_FULL_LENGTH=1 for the full-length 512^3 run")
-    case = W.tgv(512)
-    nsteps = int(os.environ.get("OSBLI_C5_STEPS", case.nsteps))
-    run_steps_case(f"tgv512_{nsteps}", case, nsteps, 1e-9, parity.q28)
+def test_config4_sbli_slab_full_length():
+    """500 RK3 steps of the curvilinear shock / boundary-layer slab, 67 200 sampled nodes, L1 <= 1e-9."""
+    run_golden_config(4)
+
+
+def test_config5_tgv512_full_length():
+    """50 RK3 steps at 512^3 (29 GB of device state), 64 000 sampled nodes, max-norm <= 1e-9."""
+    run_golden_config(5)
+
+
+def test_simple_averaging_and_ssp_rk3():
+    """simple averaging of the interface state (PAPER.md:104 step 2(a); Q38) and the
+    SSP coefficient set of the 3-stage scheme (Q39): residuals on uniform, curvilinear and
+    shocked inputs; steps through the fused update with and without periodic write-through and the 1-D path."""
+    case = W.tgv(32)
+    run_residual_case("tgv32_simple_avg_perturbed", case, Q0=W.perturb(case, seed=5, amp=0.05), averaging=W.AVG_SIMPLE)
+    run_residual_case("wavy_box_simple_avg", W.wavy_box(n=(24, 20, 8)), averaging=W.AVG_SIMPLE)
+    run_residual_case("wavy_box_simple_avg_teno6", W.wavy_box(n=(24, 20, 8), scheme=W.TENO6), averaging=W.AVG_SIMPLE)
+    sod = W.sod()
+    orc = parity.make_oracle(sod, averaging=W.AVG_SIMPLE)
+    run_residual_case("sod_t0.03_simple_avg", sod, Q0=orc.run(sod.Q0.copy(), sod.dt, 150), averaging=W.AVG_SIMPLE)
+    run_steps_case("tgv32_10_ssp", case, 10, 1e-9, parity.q28, rk3_form=W.RK3_SSP)
+    run_steps_case("tgv32_10_ssp_simple_avg", case, 10, 1e-9, parity.q28, rk3_form=W.RK3_SSP, averaging=W.AVG_SIMPLE)
+    run_steps_case("wavy_box_3_ssp", W.wavy_box(n=(40, 21, 9)), 3, 1e-9, parity.l1_rel, rk3_form=W.RK3_SSP)
+    run_steps_case("sod_300_ssp_simple_avg", sod, 300, 1e-9, parity.l1_rel, rk3_form=W.RK3_SSP, averaging=W.AVG_SIMPLE)
