@@ -40,6 +40,14 @@ from paper_2007_14933_b200 import workloads as W                 # noqa: E402
 
 GOLDEN = ROOT / "tests" / "golden"
 
+
+def use_private_library():
+    """Compile the oracle into a private temporary file for this (hours-long) process, so that a rebuild of
+    oracle/libosbli_oracle.so by a test session running meanwhile cannot touch the code being executed."""
+    import tempfile
+    O._LIB = Path(tempfile.mkdtemp(prefix="osbli_golden_")) / "libosbli_oracle_golden.so"
+    O.build(force=True)
+
 # config -> (case factory, sample stride per direction (x, y, z), checkpoints in steps)
 CONFIGS = {
     3: (lambda: W.tgv(256), (7, 7, 7), (50, 100, 200)),
@@ -78,6 +86,7 @@ def main():
     ap.add_argument("--out", type=str, default=str(GOLDEN))
     a = ap.parse_args()
 
+    use_private_library()
     make, stride, checkpoints = CONFIGS[a.config]
     case = make()
     assert checkpoints[-1] == case.nsteps, (checkpoints, case.nsteps)

@@ -14,7 +14,7 @@ CSRC = PKG / "csrc"
 LIB = PKG / "libosbli.so"
 SOURCES = ["osbli_api.cu", "osbli_sweep.cu", "osbli_visc.cu", "osbli_bc_rk.cu", "osbli_peak.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "--use_fast_math=false", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
 
 def nvcc() -> str:
@@ -35,19 +35,23 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and not needs_build():
         return LIB
-    objs = []
-    flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"]
-    flags += os.environ.get("OSBLI_NVCC_EXTRA", "").split()      # tuning experiments (-D... macros)
-    for src in SOURCES:
+    flags = NVCC_FLAGS + os.environ.get("OSBLI_NVCC_EXTRA", "").split()      # tuning experiments (-D... macros)
+
+    def compile_one(src):
         obj = CSRC / (src[:-3] + ".o")
         cmd = [nvcc(), *flags, "-c", str(CSRC / src), "-o", str(obj)]
-        res = subprocess.run(cmd, capture_output=True, text=True)
-        if verbose or res.returncode != 0:
-            sys.stderr.write(res.stdout + res.stderr)
-        if res.returncode != 0:
-            raise RuntimeError(f"nvcc failed on {src}")
-        (CSRC / (src[:-3] + ".ptxas.txt")).write_text(res.stderr)
-        objs.append(str(obj))
+        return src, obj, subprocess.run(cmd, capture_output=True, text=True)
+
+    objs = []
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as pool:
+        for src, obj, res in pool.map(compile_one, SOURCES):
+            if verbose or res.returncode != 0:
+                sys.stderr.write(res.stdout + res.stderr)
+            if res.returncode != 0:
+                raise RuntimeError(f"nvcc failed on {src}")
+            (CSRC / (src[:-3] + ".ptxas.txt")).write_text(res.stderr)
+            objs.append(str(obj))
     tmp = LIB.with_suffix(f".tmp{os.getpid()}.so")
     cmd = [nvcc(), "-shared", "-o", str(tmp), *objs]
     subprocess.run(cmd, check=True)

@@ -21,6 +21,7 @@ struct osbli_ctx {
   int64_t launches;
   bool profiling;
   std::vector<ProfiledLaunch> *prof;   // events around every launch while profiling
+  TmapCache tmaps;                     // tensor maps of the states seen by the fast viscous kernel
 };
 
 namespace {
@@ -99,7 +100,8 @@ inline cudaStream_t as_stream(void *s) { return reinterpret_cast<cudaStream_t>(s
   do {                                                                   \
     ProfiledLaunch pl_ = {cls, nullptr, nullptr};                        \
     if ((h)->profiling) {                                                \
-      if (cudaEventCreate(&pl_.t0) != cudaSuccess || cudaEventCreate(&pl_.t1) != cudaSuccess) return OSBLI_ECUDA; \
+      if (cudaEventCreate(&pl_.t0) != cudaSuccess) return OSBLI_ECUDA;   \
+      if (cudaEventCreate(&pl_.t1) != cudaSuccess) { cudaEventDestroy(pl_.t0); return OSBLI_ECUDA; } \
       cudaEventRecord(pl_.t0, st);                                       \
     }                                                                    \
     if ((call) != cudaSuccess) return OSBLI_ECUDA;                       \
@@ -123,7 +125,7 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
   if (P.scheme == OSBLI_SCHEME_CENTRAL4) {                            // no sweeps: central convective terms, then the rest
     if (rk) return OSBLI_EINVAL;
     OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X, st, launch_central(P, Q, R, st));
-    if (fast_visc) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous_fast(P, Q, R, st));
+    if (fast_visc) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous_fast(P, Q, R, &h->tmaps, st));
     else if (P.visc != OSBLI_VISC_NONE) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, 1, st));
     if (P.has_force) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_force(P, Q, R, st));
     return OSBLI_OK;
@@ -135,7 +137,7 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
   for (int d = 0; d < 3; ++d) {
     if (P.L.n[d] <= 1) continue;
     if (d == last && last > 0) {                                    // viscous terms go in front of the last sweep
-      if (fast_visc) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous_fast(P, Q, R, st));
+      if (fast_visc) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous_fast(P, Q, R, &h->tmaps, st));
       else if (P.visc != OSBLI_VISC_NONE) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, accumulate, st));
       if (P.has_force) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_force(P, Q, R, st));
     }
@@ -214,6 +216,8 @@ int osbli_init(const osbli_params *p, void *d_workspace, size_t workspace_bytes,
   cudaDeviceProp prop;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return OSBLI_ECUDA;
   if (prop.major != 10) return OSBLI_ECUDA;                      // sm_100a code only; no other path exists
+  // opt-in shared-memory sizes are per device: set them for the device this handle lives on
+  if (sweep_set_attributes() != cudaSuccess || viscous_set_attributes() != cudaSuccess) return OSBLI_ECUDA;
 
   osbli_ctx *h = new (std::nothrow) osbli_ctx;
   if (!h) return OSBLI_EINVAL;

@@ -22,7 +22,17 @@ cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *pr
 
 // fused fast path (uniform grid, mu = 1, three periodic directions): reads Q directly, R += viscous terms
 bool viscous_fast_path(const DevParams &P);
-cudaError_t launch_viscous_fast(const DevParams &P, const double *Q, double *R, cudaStream_t st);
+struct TmapCache {                    // tensor maps of the states the fast viscous kernel has been launched on (host side)
+  static constexpr int kSlots = 4;
+  struct alignas(64) Map { unsigned long long opaque[16]; } map[kSlots];   // CUtensorMap (128 bytes, 64-byte aligned)
+  const double *ptr[kSlots];
+  int count, next;
+};
+cudaError_t launch_viscous_fast(const DevParams &P, const double *Q, double *R, TmapCache *cache, cudaStream_t st);
+
+// Per-device one-time set-up (opt-in dynamic shared-memory sizes): called by osbli_init for the current device.
+cudaError_t sweep_set_attributes();
+cudaError_t viscous_set_attributes();
 
 // central convective terms, scheme 4 (osbli_visc.cu): R = - sum_d delta_d F_d on interior nodes (writes R)
 cudaError_t launch_central(const DevParams &P, const double *Q, double *R, cudaStream_t st);

@@ -365,12 +365,6 @@ static cudaError_t launch_x(const DevParams &P, const double *Q, double *R, int 
   if (nx <= 64) chunk = ((nx + kXT - 1) / kXT) * kXT;
   dim3 grid((nlines + kXWarps * 32 - 1) / (kXWarps * 32), (nx + chunk - 1) / chunk, 1);
   const size_t smem = sizeof(XSmem<CURV>) * kXWarps;
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaError_t e = cudaFuncSetAttribute(sweep_x_kernel<SCHEME, CURV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    attr_done = true;
-  }
   sweep_x_kernel<SCHEME, CURV><<<grid, kXWarps * 32, smem, st>>>(P, Q, R, chunk, accumulate);
   return cudaGetLastError();
 }
@@ -394,6 +388,22 @@ static cudaError_t launch_yz(const DevParams &P, const double *Q, double *R, int
   } else if (accumulate) sweep_yz_kernel<DIR, SCHEME, CURV, true, 0><<<grid, bx, 0, st>>>(P, Q, R, chunk, none);
   else sweep_yz_kernel<DIR, SCHEME, CURV, false, 0><<<grid, bx, 0, st>>>(P, Q, R, chunk, none);
   return cudaGetLastError();
+}
+
+// Opt-in dynamic shared memory of every x-sweep instantiation, for the current device (osbli_init).
+template <int SCHEME, bool CURV>
+static cudaError_t set_x_attr() {
+  return cudaFuncSetAttribute(sweep_x_kernel<SCHEME, CURV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)(sizeof(XSmem<CURV>) * kXWarps));
+}
+cudaError_t sweep_set_attributes() {
+  cudaError_t e;
+#define OSBLI_ATTR(SCH) \
+  if ((e = set_x_attr<SCH, false>()) != cudaSuccess) return e; \
+  if ((e = set_x_attr<SCH, true>()) != cudaSuccess) return e;
+  OSBLI_ATTR(0) OSBLI_ATTR(1) OSBLI_ATTR(2) OSBLI_ATTR(3) OSBLI_ATTR(5)
+#undef OSBLI_ATTR
+  return cudaSuccess;
 }
 
 cudaError_t launch_sweep(const DevParams &P, int dir, const double *Q, double *R, int accumulate, const RkArgs *rk,

@@ -298,28 +298,39 @@ cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *pr
 // =============================================================================================
 // Fast path: uniform grid, mu = 1, three active periodic directions (the Taylor-Green cases).
 //
-// 2.5-D marching: a block owns a 32 x 8 (x,y) tile and walks along z.  Each new z-plane of
-// u, v, w, T (tile + 2-deep x/y halo, computed from Q on the fly: no staged primitive arrays, no
-// extra HBM pass) goes into a 4-slot shared-memory ring; a thread keeps 5-deep z-windows of its own
-// column in registers: u, v, w, T for the z-derivatives, and d_x u, d_y v, d_x w, d_y w so that the
-// x-z / y-z mixed derivatives are z-differences of its own registers.  Only the x-y mixed
-// derivatives and the in-plane stencils read shared memory (84 LDS.64 per node).  One barrier per
-// plane.  The raw planes arrive by TMA two steps ahead of their use, R of the node by cp.async into a
-// per-thread slot: nothing waits in registers.
+// 2.5-D marching: a block owns a 32 x 8 (x,y) tile and walks along z.  The kernel is bound by the
+// shared-memory data path (every in-plane stencil value is an LDS), so every in-plane stencil is read
+// exactly ONCE, when its plane enters the pipeline (two steps before it becomes the centre plane):
+//   * raw plane tiles (36 x 12 x 5 variables) arrive by TMA two steps ahead (4-D tensor map, mbarrier),
+//     are turned into u, v, w, T planes in a 2-slot shared-memory ring (the plane being staged and the
+//     plane entering);
+//   * on entry a thread reads the x- and y-stencils of its node (32 LDS) and forms every in-plane first and
+//     second difference at once; what the centre step will need of them waits in registers: z-windows of
+//     u, v, w and of S0 = d_x w, S1 = d_y w, S2 = d_x u + d_y v (whose z-differences are the x-z / y-z
+//     mixed terms of d_i(div u)), the in-plane parts of the three momentum operators (3-deep delay
+//     lines), and 5-deep scatter accumulators of the energy equation's linear + in-plane part;
+//   * the x-y mixed differences d_x(d_y u), d_x(d_y v) come from a small exchange buffer: each thread
+//     publishes d_y u, d_y v of its node (one warp adds the 2-deep x halo columns) and reads its four
+//     x-neighbours one step later -- 8 LDS instead of the 32 of a direct 16-point evaluation.
+// 44 LDS.64 per node instead of 84; one barrier per plane; R of the node travels by cp.async into a
+// per-thread slot.
 // =============================================================================================
 #ifndef OSBLI_VCHUNK
 #define OSBLI_VCHUNK 32
 #endif
+#ifndef OSBLI_VMINB
+#define OSBLI_VMINB 2
+#endif
 constexpr int kVX = 32, kVY = 8, kVH = 2;
 constexpr int kVPX = kVX + 2 * kVH, kVPY = kVY + 2 * kVH;        // 36 x 12 plane tile
-constexpr int kVRing = 4;
 
 // Raw planes reach shared memory by TMA: the 36 x 12 tile of all five variables of one plane is one box of a
 // 4-D tensor map over the state, loaded by one cp.async.bulk.tensor issued by one thread, completion on an
 // mbarrier; rows and columns past the array are zero-filled by the hardware (ragged tiles need no guards).
 struct VSmem {
   double tile[2][5][kVPY][kVPX];       // TMA destinations (128-byte aligned: first member), double buffered
-  double f[kVRing][4][kVPY][kVPX];     // ring of u, v, w, T planes (tile + 2-deep x/y halo)
+  double f[2][4][kVPY][kVPX];          // u, v, w, T: the plane being staged and the plane entering
+  double g[2][2][kVY][kVPX];           // d_y u, d_y v of the tile rows incl. the x halo, double buffered
   double r[4][kVX * kVY];              // per-thread slots: R of the node in flight (cp.async)
   unsigned long long mbar[2];          // one mbarrier per TMA buffer
 };
@@ -349,7 +360,7 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, i
                ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
 }
 
-__global__ void __launch_bounds__(kVX * kVY, 2)
+__global__ void __launch_bounds__(kVX * kVY, OSBLI_VMINB)
 viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
                    int chunk, const __grid_constant__ CUtensorMap tmap) {
   extern __shared__ __align__(128) unsigned char vs_raw[];
@@ -385,7 +396,7 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
     }
   };
   auto stage = [&](int plane) {
-    const int slot = (plane + 8) & (kVRing - 1);
+    const int slot = (plane + 8) & 1;
     const int jj = plane - (z0 - 2), b = jj & 1;
     mbar_wait(&S.mbar[b], (unsigned)(jj >> 1) & 1u);
 #pragma unroll
@@ -415,27 +426,33 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
   auto d2 = [](double m2, double m1, double f0, double p1, double p2, double c) {
     return c * fma(-30.0, f0, fma(16.0, m1 + p1, -(m2 + p2)));
   };
+  constexpr double third = 1.0 / 3.0, four3 = 4.0 / 3.0;
 
-  double uw[5], vw[5], ww[5], Tw[5], uxw[5], vyw[5], wxw[5], wyw[5];
+  // register state of this thread's column.  After the shift of step k: windows hold planes k-2..k+2, delay
+  // lines planes k..k+2, the energy accumulators planes k..k+4.
+  double uw[5], vw[5], ww[5], s0w[5], s1w[5], s2w[5];
+  double Au[3], Av[3], Aw[3];        // in-plane parts of M_0, M_1, M_2 (incl. the x-y mixed terms, folded one step later)
+  double aE[5];                      // cq (T_xx + T_yy + T_zz) + (2 u_x^2 + 2 v_y^2 + (u_y + v_x)^2)/Re, scatter form
 #pragma unroll
-  for (int m = 0; m < 5; ++m) uw[m] = vw[m] = ww[m] = Tw[m] = uxw[m] = vyw[m] = wxw[m] = wyw[m] = 0.0;
+  for (int m = 0; m < 5; ++m) uw[m] = vw[m] = ww[m] = s0w[m] = s1w[m] = s2w[m] = aE[m] = 0.0;
+#pragma unroll
+  for (int m = 0; m < 3; ++m) Au[m] = Av[m] = Aw[m] = 0.0;
 
-  // Software pipeline, one barrier per plane: during step k (node k is finished) plane k+3 is
-  // staged into the slot plane k-1 has just left, plane k+4 is fetched into registers, plane k+2
-  // (staged one step earlier) enters the register windows and plane k is the centre of the
-  // in-plane stencils -- so staging, global loads and the stencil arithmetic of a step are
-  // independent of each other and the barrier closes the step.
+  // Software pipeline, one barrier per plane: during step k (node k is finished) plane k+3 is staged into
+  // the ring slot plane k+1 has left, the raw plane k+4 is fetched, plane k+2 (staged one step earlier)
+  // enters, the x-y mixed terms of plane k+1 are folded in, and plane k is completed from registers alone.
   fetch(z0 - 2);
   stage(z0 - 2);
   fetch(z0 - 1);
   __syncthreads();
   const int X = tx + kVH, Y = ty + kVH;
+  // the warp that also publishes d_y u, d_y v of the x halo columns: 8 rows x 4 columns
+  const int hr = tid >> 2, hc = (tid & 3) < 2 ? (tid & 3) : kVX + (tid & 3);
 
   for (int k = z0 - 4; k < z1; ++k) {
     if (k > z0 - 4) __syncthreads();
     if (k + 3 < z1 + 2) stage(k + 3);
-    // R of node k goes to a per-thread shared-memory slot by cp.async (held in registers it was spilled
-    // right behind the load, a full-latency stall)
+    // R of node k goes to a per-thread shared-memory slot by cp.async
     long long at = 0;
     if (k >= z0 && inside) {
       at = L.at(i, j, k);
@@ -446,73 +463,72 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
     if (k + 4 < z1 + 2) fetch(k + 4);                          // raw plane k+4 into the buffer plane k+2 has left
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
-      uw[m] = uw[m + 1]; vw[m] = vw[m + 1]; ww[m] = ww[m + 1]; Tw[m] = Tw[m + 1];
-      uxw[m] = uxw[m + 1]; vyw[m] = vyw[m + 1]; wxw[m] = wxw[m + 1]; wyw[m] = wyw[m + 1];
+      uw[m] = uw[m + 1]; vw[m] = vw[m + 1]; ww[m] = ww[m + 1];
+      s0w[m] = s0w[m + 1]; s1w[m] = s1w[m + 1]; s2w[m] = s2w[m + 1]; aE[m] = aE[m + 1];
+    }
+    aE[4] = 0.0;
+    Au[0] = Au[1]; Au[1] = Au[2]; Av[0] = Av[1]; Av[1] = Av[2]; Aw[0] = Aw[1]; Aw[1] = Aw[2];
+    {
+      // ---- plane k+2 enters: every in-plane stencil of this node, read once
+      const int e = (k + 2 + 8) & 1;
+      const double (*F)[kVPY][kVPX] = S.f[e];
+      const double u = F[0][Y][X], v = F[1][Y][X], w = F[2][Y][X], T = F[3][Y][X];
+      const double uxm2 = F[0][Y][X - 2], uxm1 = F[0][Y][X - 1], uxp1 = F[0][Y][X + 1], uxp2 = F[0][Y][X + 2];
+      const double uym2 = F[0][Y - 2][X], uym1 = F[0][Y - 1][X], uyp1 = F[0][Y + 1][X], uyp2 = F[0][Y + 2][X];
+      const double u_x = d1(uxm2, uxm1, uxp1, uxp2, cx), u_y = d1(uym2, uym1, uyp1, uyp2, cy);
+      Au[2] = fma(four3, d2(uxm2, uxm1, u, uxp1, uxp2, cxx), d2(uym2, uym1, u, uyp1, uyp2, cyy));
+      const double vxm2 = F[1][Y][X - 2], vxm1 = F[1][Y][X - 1], vxp1 = F[1][Y][X + 1], vxp2 = F[1][Y][X + 2];
+      const double vym2 = F[1][Y - 2][X], vym1 = F[1][Y - 1][X], vyp1 = F[1][Y + 1][X], vyp2 = F[1][Y + 2][X];
+      const double v_x = d1(vxm2, vxm1, vxp1, vxp2, cx), v_y = d1(vym2, vym1, vyp1, vyp2, cy);
+      Av[2] = fma(four3, d2(vym2, vym1, v, vyp1, vyp2, cyy), d2(vxm2, vxm1, v, vxp1, vxp2, cxx));
+      S.g[e][0][ty][X] = u_y;
+      S.g[e][1][ty][X] = v_y;
+      const double wxm2 = F[2][Y][X - 2], wxm1 = F[2][Y][X - 1], wxp1 = F[2][Y][X + 1], wxp2 = F[2][Y][X + 2];
+      const double wym2 = F[2][Y - 2][X], wym1 = F[2][Y - 1][X], wyp1 = F[2][Y + 1][X], wyp2 = F[2][Y + 2][X];
+      Aw[2] = d2(wxm2, wxm1, w, wxp1, wxp2, cxx) + d2(wym2, wym1, w, wyp1, wyp2, cyy);
+      const double lapT = d2(F[3][Y][X - 2], F[3][Y][X - 1], T, F[3][Y][X + 1], F[3][Y][X + 2], cxx) +
+                          d2(F[3][Y - 2][X], F[3][Y - 1][X], T, F[3][Y + 1][X], F[3][Y + 2][X], cyy);
+      uw[4] = u; vw[4] = v; ww[4] = w;
+      s0w[4] = d1(wxm2, wxm1, wxp1, wxp2, cx);
+      s1w[4] = d1(wym2, wym1, wyp1, wyp2, cy);
+      s2w[4] = u_x + v_y;
+      // energy equation, everything that is linear in plane k+2 or lives in it: the z-stencil of T scattered to
+      // the five planes it feeds (accumulator m <-> plane k+m, stencil offset 2-m), plus the in-plane terms
+      const double sxy = u_y + v_x;
+      const double tz = (P.cq * czz) * T;
+      aE[0] -= tz; aE[1] = fma(16.0, tz, aE[1]); aE[3] = fma(16.0, tz, aE[3]); aE[4] -= tz;
+      aE[2] = fma(-30.0, tz, aE[2]) + fma(P.cq, lapT, P.inv_Re * fma(sxy, sxy, 2.0 * fma(u_x, u_x, v_y * v_y)));
+      if (tid < 32) {                                            // x halo columns of the exchange buffer
+        const int Yh = hr + kVH;
+        S.g[e][0][hr][hc] = d1(F[0][Yh - 2][hc], F[0][Yh - 1][hc], F[0][Yh + 1][hc], F[0][Yh + 2][hc], cy);
+        S.g[e][1][hr][hc] = d1(F[1][Yh - 2][hc], F[1][Yh - 1][hc], F[1][Yh + 1][hc], F[1][Yh + 2][hc], cy);
+      }
     }
     {
-      const double (*F)[kVPY][kVPX] = S.f[(k + 2 + 8) & (kVRing - 1)];      // plane k+2
-      uw[4] = F[0][Y][X]; vw[4] = F[1][Y][X]; ww[4] = F[2][Y][X]; Tw[4] = F[3][Y][X];
-      uxw[4] = d1(F[0][Y][X - 2], F[0][Y][X - 1], F[0][Y][X + 1], F[0][Y][X + 2], cx);
-      wxw[4] = d1(F[2][Y][X - 2], F[2][Y][X - 1], F[2][Y][X + 1], F[2][Y][X + 2], cx);
-      vyw[4] = d1(F[1][Y - 2][X], F[1][Y - 1][X], F[1][Y + 1][X], F[1][Y + 2][X], cy);
-      wyw[4] = d1(F[2][Y - 2][X], F[2][Y - 1][X], F[2][Y + 1][X], F[2][Y + 2][X], cy);
+      // ---- x-y mixed terms of plane k+1: d_x of the d_y values published one step ago
+      const double (*G)[kVY][kVPX] = S.g[(k + 1 + 8) & 1];
+      Au[1] = fma(third, d1(G[1][ty][X - 2], G[1][ty][X - 1], G[1][ty][X + 1], G[1][ty][X + 2], cx), Au[1]);   // + v_xy / 3
+      Av[1] = fma(third, d1(G[0][ty][X - 2], G[0][ty][X - 1], G[0][ty][X + 1], G[0][ty][X + 2], cx), Av[1]);   // + u_xy / 3
     }
     if (k < z0 || !inside) continue;
 
-    const double (*F)[kVPY][kVPX] = S.f[(k + 8) & (kVRing - 1)];
-    // in-plane stencils of the current plane
-    const double u = uw[2], v = vw[2], w = ww[2], T = Tw[2];
-    const double uxm2 = F[0][Y][X - 2], uxm1 = F[0][Y][X - 1], uxp1 = F[0][Y][X + 1], uxp2 = F[0][Y][X + 2];
-    const double uym2 = F[0][Y - 2][X], uym1 = F[0][Y - 1][X], uyp1 = F[0][Y + 1][X], uyp2 = F[0][Y + 2][X];
-    const double vxm2 = F[1][Y][X - 2], vxm1 = F[1][Y][X - 1], vxp1 = F[1][Y][X + 1], vxp2 = F[1][Y][X + 2];
-    const double vym2 = F[1][Y - 2][X], vym1 = F[1][Y - 1][X], vyp1 = F[1][Y + 1][X], vyp2 = F[1][Y + 2][X];
-    const double u_x = uxw[2], v_y = vyw[2], w_x = wxw[2], w_y = wyw[2];
-    const double u_y = d1(uym2, uym1, uyp1, uyp2, cy);
-    const double v_x = d1(vxm2, vxm1, vxp1, vxp2, cx);
+    // ---- plane k is complete: z-direction terms from the register windows
+    const double u = uw[2], v = vw[2], w = ww[2];
     const double u_z = d1(uw[0], uw[1], uw[3], uw[4], cz);
     const double v_z = d1(vw[0], vw[1], vw[3], vw[4], cz);
     const double w_z = d1(ww[0], ww[1], ww[3], ww[4], cz);
-    const double u_xx = d2(uxm2, uxm1, u, uxp1, uxp2, cxx), u_yy = d2(uym2, uym1, u, uyp1, uyp2, cyy);
-    const double v_xx = d2(vxm2, vxm1, v, vxp1, vxp2, cxx), v_yy = d2(vym2, vym1, v, vyp1, vyp2, cyy);
     const double u_zz = d2(uw[0], uw[1], u, uw[3], uw[4], czz);
     const double v_zz = d2(vw[0], vw[1], v, vw[3], vw[4], czz);
     const double w_zz = d2(ww[0], ww[1], w, ww[3], ww[4], czz);
-    const double w_xx = d2(F[2][Y][X - 2], F[2][Y][X - 1], w, F[2][Y][X + 1], F[2][Y][X + 2], cxx);
-    const double w_yy = d2(F[2][Y - 2][X], F[2][Y - 1][X], w, F[2][Y + 1][X], F[2][Y + 2][X], cyy);
-    const double T_xx = d2(F[3][Y][X - 2], F[3][Y][X - 1], T, F[3][Y][X + 1], F[3][Y][X + 2], cxx);
-    const double T_yy = d2(F[3][Y - 2][X], F[3][Y - 1][X], T, F[3][Y + 1][X], F[3][Y + 2][X], cyy);
-    const double T_zz = d2(Tw[0], Tw[1], T, Tw[3], Tw[4], czz);
-    // x-y mixed: delta_x (delta_y f), 16 points each
-    auto dxy = [&](int f) {
-      const double a2 = d1(F[f][Y - 2][X - 2], F[f][Y - 1][X - 2], F[f][Y + 1][X - 2], F[f][Y + 2][X - 2], cy);
-      const double a1 = d1(F[f][Y - 2][X - 1], F[f][Y - 1][X - 1], F[f][Y + 1][X - 1], F[f][Y + 2][X - 1], cy);
-      const double b1 = d1(F[f][Y - 2][X + 1], F[f][Y - 1][X + 1], F[f][Y + 1][X + 1], F[f][Y + 2][X + 1], cy);
-      const double b2 = d1(F[f][Y - 2][X + 2], F[f][Y - 1][X + 2], F[f][Y + 1][X + 2], F[f][Y + 2][X + 2], cy);
-      return d1(a2, a1, b1, b2, cx);
-    };
-    const double u_xy = dxy(0), v_xy = dxy(1);
-    const double u_xz = d1(uxw[0], uxw[1], uxw[3], uxw[4], cz);
-    const double w_xz = d1(wxw[0], wxw[1], wxw[3], wxw[4], cz);
-    const double v_yz = d1(vyw[0], vyw[1], vyw[3], vyw[4], cz);
-    const double w_yz = d1(wyw[0], wyw[1], wyw[3], wyw[4], cz);
-
-    const double div = u_x + v_y + w_z;
-    const double third = 1.0 / 3.0;
-    const double M0 = fma(third, u_xx + v_xy + w_xz, u_xx + u_yy + u_zz);
-    const double M1 = fma(third, u_xy + v_yy + w_yz, v_xx + v_yy + v_zz);
-    const double M2 = fma(third, u_xz + v_yz + w_zz, w_xx + w_yy + w_zz);
-    // tau_ij d_j u_i with tau = (d_j u_i + d_i u_j - 2/3 delta_ij div)/Re
-    const double t23 = (2.0 / 3.0) * div;
-    const double sxy = u_y + v_x, sxz = u_z + w_x, syz = v_z + w_y;
-    double phi = (2.0 * u_x - t23) * u_x;
-    phi = fma(2.0 * v_y - t23, v_y, phi);
-    phi = fma(2.0 * w_z - t23, w_z, phi);
-    phi = fma(sxy, sxy, phi);
-    phi = fma(sxz, sxz, phi);
-    phi = fma(syz, syz, phi);
-    const double heat = P.cq * (T_xx + T_yy + T_zz);
+    const double M0 = Au[0] + fma(third, d1(s0w[0], s0w[1], s0w[3], s0w[4], cz), u_zz);          // + w_xz / 3
+    const double M1 = Av[0] + fma(third, d1(s1w[0], s1w[1], s1w[3], s1w[4], cz), v_zz);          // + w_yz / 3
+    const double M2 = Aw[0] + fma(third, d1(s2w[0], s2w[1], s2w[3], s2w[4], cz), four3 * w_zz);  // + (u_xz + v_yz)/3
+    // tau_ij d_j u_i = [2 (u_x^2 + v_y^2 + w_z^2) - 2/3 div^2 + s_xy^2 + s_xz^2 + s_yz^2]/Re; the in-plane part is in aE
+    const double div = s2w[2] + w_z;
+    const double sxz = u_z + s0w[2], syz = v_z + s1w[2];
+    const double phiz = fma(sxz, sxz, fma(syz, syz, fma(2.0 * w_z, w_z, (-2.0 / 3.0) * (div * div))));
     const double r1 = M0 * P.inv_Re, r2 = M1 * P.inv_Re, r3 = M2 * P.inv_Re;
-    const double r4 = fma(u, r1, fma(v, r2, w * r3)) + fma(phi, P.inv_Re, heat);
+    const double r4 = fma(u, r1, fma(v, r2, w * r3)) + fma(phiz, P.inv_Re, aE[0]);
     asm volatile("cp.async.wait_all;" ::: "memory");           // R has landed
     const double rold[4] = {S.r[0][tid], S.r[1][tid], S.r[2][tid], S.r[3][tid]};
     R[sv + at] = rold[0] + r1;
@@ -556,20 +572,28 @@ static bool encode_state_map(const Layout &L, const double *Q, CUtensorMap *map)
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-cudaError_t launch_viscous_fast(const DevParams &P, const double *Q, double *R, cudaStream_t st) {
+// The tensor map depends on the state's base address only; the step cycles through three states (Q, Q2, Q3), so
+// the handle keeps a small cache and the driver's encoder runs once per address instead of once per launch.
+cudaError_t launch_viscous_fast(const DevParams &P, const double *Q, double *R, TmapCache *cache, cudaStream_t st) {
   const Layout &L = P.L;
   const int chunk = L.n[2] > OSBLI_VCHUNK ? OSBLI_VCHUNK : L.n[2];
   dim3 grid((L.n[0] + kVX - 1) / kVX, (L.n[1] + kVY - 1) / kVY, (L.n[2] + chunk - 1) / chunk);
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaError_t e = cudaFuncSetAttribute(viscous_tgv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(VSmem));
-    if (e != cudaSuccess) return e;
-    attr_done = true;
+  static_assert(sizeof(CUtensorMap) == sizeof(cache->map[0]), "TmapCache::map must hold a CUtensorMap");
+  int hit = -1;
+  for (int e = 0; e < cache->count; ++e)
+    if (cache->ptr[e] == Q) hit = e;
+  if (hit < 0) {
+    hit = cache->count < TmapCache::kSlots ? cache->count++ : (cache->next++ % TmapCache::kSlots);
+    if (!encode_state_map(L, Q, reinterpret_cast<CUtensorMap *>(&cache->map[hit]))) { cache->count = 0; return cudaErrorNotSupported; }
+    cache->ptr[hit] = Q;
   }
-  CUtensorMap map;
-  if (!encode_state_map(L, Q, &map)) return cudaErrorNotSupported;
-  viscous_tgv_kernel<<<grid, dim3(kVX, kVY), sizeof(VSmem), st>>>(P, Q, R, chunk, map);
+  viscous_tgv_kernel<<<grid, dim3(kVX, kVY), sizeof(VSmem), st>>>(P, Q, R, chunk, *reinterpret_cast<const CUtensorMap *>(&cache->map[hit]));
   return cudaGetLastError();
+}
+
+// Opt-in shared-memory sizes of the kernels of this file, once per device (called by osbli_init).
+cudaError_t viscous_set_attributes() {
+  return cudaFuncSetAttribute(viscous_tgv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(VSmem));
 }
 
 }  // namespace osbli
