@@ -9,7 +9,8 @@
 // adding  d_j tau_ij,  d_j(u_i tau_ij) - d_j q_j  to R.
 #include "osbli_kernels.h"
 
-#include <cuda.h>          // CUtensorMap (types only; the encoder is fetched through the runtime)
+#include <cuda.h>
+#include <type_traits>          // CUtensorMap (types only; the encoder is fetched through the runtime)
 
 namespace osbli {
 
@@ -331,7 +332,7 @@ struct VSmem {
   double tile[2][5][kVPY][kVPX];       // TMA destinations (128-byte aligned: first member), double buffered
   double f[2][4][kVPY][kVPX];          // u, v, w, T: the plane being staged and the plane entering
   double g[2][2][kVY][kVPX];           // d_y u, d_y v of the tile rows incl. the x halo, double buffered
-  double r[4][kVX * kVY];              // per-thread slots: R of the node in flight (cp.async)
+  double r[2][4][kVX * kVY];           // per-thread slots: R of the two nodes in flight (cp.async, issued one step ahead)
   unsigned long long mbar[2];          // one mbarrier per TMA buffer
 };
 constexpr unsigned kVTileBytes = 5 * kVPY * kVPX * sizeof(double);
@@ -428,8 +429,9 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
   };
   constexpr double third = 1.0 / 3.0, four3 = 4.0 / 3.0;
 
-  // register state of this thread's column.  After the shift of step k: windows hold planes k-2..k+2, delay
-  // lines planes k..k+2, the energy accumulators planes k..k+4.
+  // Register state of this thread's column.  After the shift of step k: windows hold planes k-2..k+2 (slots
+  // 0..4), the delay lines planes k..k+2 (slots 0..2), the energy accumulators planes k..k+4.  (Unrolling the plane loop five times so that the windows rotate without
+  // register moves was measured: 0.467 -> 0.492 ms, 66 KB of code against a 32 KB instruction cache.)
   double uw[5], vw[5], ww[5], s0w[5], s1w[5], s2w[5];
   double Au[3], Av[3], Aw[3];        // in-plane parts of M_0, M_1, M_2 (incl. the x-y mixed terms, folded one step later)
   double aE[5];                      // cq (T_xx + T_yy + T_zz) + (2 u_x^2 + 2 v_y^2 + (u_y + v_x)^2)/Re, scatter form
@@ -449,15 +451,16 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
   // the warp that also publishes d_y u, d_y v of the x halo columns: 8 rows x 4 columns
   const int hr = tid >> 2, hc = (tid & 3) < 2 ? (tid & 3) : kVX + (tid & 3);
 
+  constexpr int M2 = 0, M1 = 1, C = 2, P1 = 3, P2 = 4;          // window slots of planes k-2, k-1, k, k+1, k+2
   for (int k = z0 - 4; k < z1; ++k) {
     if (k > z0 - 4) __syncthreads();
     if (k + 3 < z1 + 2) stage(k + 3);
-    // R of node k goes to a per-thread shared-memory slot by cp.async
-    long long at = 0;
-    if (k >= z0 && inside) {
-      at = L.at(i, j, k);
+    // R of node k+1 goes to a per-thread shared-memory slot by cp.async, one whole step before it is needed (the
+    // arithmetic of a single step does not cover the DRAM latency)
+    if (k + 1 >= z0 && k + 1 < z1 && inside) {
+      const long long a1 = L.at(i, j, k + 1);
 #pragma unroll
-      for (int c = 0; c < 4; ++c) cp_async8(&S.r[c][tid], R + (c + 1) * sv + at);
+      for (int c = 0; c < 4; ++c) cp_async8(&S.r[(k + 1) & 1][c][tid], R + (c + 1) * sv + a1);
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
     if (k + 4 < z1 + 2) fetch(k + 4);                          // raw plane k+4 into the buffer plane k+2 has left
@@ -468,43 +471,49 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
     }
     aE[4] = 0.0;
     Au[0] = Au[1]; Au[1] = Au[2]; Av[0] = Av[1]; Av[1] = Av[2]; Aw[0] = Aw[1]; Aw[1] = Aw[2];
-    {
-      // ---- plane k+2 enters: every in-plane stencil of this node, read once
+    // ---- plane k+2 enters: every in-plane stencil of this node, read once.  The two planes either side of the
+    // chunk only feed z-stencils: they need u, v, w, T, S0, S1, S2 and nothing else (FULL = false).
+    auto enter = [&](auto full_tag) {
+      constexpr bool FULL = decltype(full_tag)::value;
       const int e = (k + 2 + 8) & 1;
       const double (*F)[kVPY][kVPX] = S.f[e];
       const double u = F[0][Y][X], v = F[1][Y][X], w = F[2][Y][X], T = F[3][Y][X];
       const double uxm2 = F[0][Y][X - 2], uxm1 = F[0][Y][X - 1], uxp1 = F[0][Y][X + 1], uxp2 = F[0][Y][X + 2];
-      const double uym2 = F[0][Y - 2][X], uym1 = F[0][Y - 1][X], uyp1 = F[0][Y + 1][X], uyp2 = F[0][Y + 2][X];
-      const double u_x = d1(uxm2, uxm1, uxp1, uxp2, cx), u_y = d1(uym2, uym1, uyp1, uyp2, cy);
-      Au[2] = fma(four3, d2(uxm2, uxm1, u, uxp1, uxp2, cxx), d2(uym2, uym1, u, uyp1, uyp2, cyy));
-      const double vxm2 = F[1][Y][X - 2], vxm1 = F[1][Y][X - 1], vxp1 = F[1][Y][X + 1], vxp2 = F[1][Y][X + 2];
       const double vym2 = F[1][Y - 2][X], vym1 = F[1][Y - 1][X], vyp1 = F[1][Y + 1][X], vyp2 = F[1][Y + 2][X];
-      const double v_x = d1(vxm2, vxm1, vxp1, vxp2, cx), v_y = d1(vym2, vym1, vyp1, vyp2, cy);
-      Av[2] = fma(four3, d2(vym2, vym1, v, vyp1, vyp2, cyy), d2(vxm2, vxm1, v, vxp1, vxp2, cxx));
-      S.g[e][0][ty][X] = u_y;
-      S.g[e][1][ty][X] = v_y;
       const double wxm2 = F[2][Y][X - 2], wxm1 = F[2][Y][X - 1], wxp1 = F[2][Y][X + 1], wxp2 = F[2][Y][X + 2];
       const double wym2 = F[2][Y - 2][X], wym1 = F[2][Y - 1][X], wyp1 = F[2][Y + 1][X], wyp2 = F[2][Y + 2][X];
-      Aw[2] = d2(wxm2, wxm1, w, wxp1, wxp2, cxx) + d2(wym2, wym1, w, wyp1, wyp2, cyy);
-      const double lapT = d2(F[3][Y][X - 2], F[3][Y][X - 1], T, F[3][Y][X + 1], F[3][Y][X + 2], cxx) +
-                          d2(F[3][Y - 2][X], F[3][Y - 1][X], T, F[3][Y + 1][X], F[3][Y + 2][X], cyy);
-      uw[4] = u; vw[4] = v; ww[4] = w;
-      s0w[4] = d1(wxm2, wxm1, wxp1, wxp2, cx);
-      s1w[4] = d1(wym2, wym1, wyp1, wyp2, cy);
-      s2w[4] = u_x + v_y;
+      const double u_x = d1(uxm2, uxm1, uxp1, uxp2, cx), v_y = d1(vym2, vym1, vyp1, vyp2, cy);
+      uw[P2] = u; vw[P2] = v; ww[P2] = w;
+      s0w[P2] = d1(wxm2, wxm1, wxp1, wxp2, cx);
+      s1w[P2] = d1(wym2, wym1, wyp1, wyp2, cy);
+      s2w[P2] = u_x + v_y;
       // energy equation, everything that is linear in plane k+2 or lives in it: the z-stencil of T scattered to
-      // the five planes it feeds (accumulator m <-> plane k+m, stencil offset 2-m), plus the in-plane terms
-      const double sxy = u_y + v_x;
+      // the five planes k..k+4 it feeds (weights -1, 16, -30, 16, -1), plus the in-plane terms
       const double tz = (P.cq * czz) * T;
-      aE[0] -= tz; aE[1] = fma(16.0, tz, aE[1]); aE[3] = fma(16.0, tz, aE[3]); aE[4] -= tz;
-      aE[2] = fma(-30.0, tz, aE[2]) + fma(P.cq, lapT, P.inv_Re * fma(sxy, sxy, 2.0 * fma(u_x, u_x, v_y * v_y)));
-      if (tid < 32) {                                            // x halo columns of the exchange buffer
-        const int Yh = hr + kVH;
-        S.g[e][0][hr][hc] = d1(F[0][Yh - 2][hc], F[0][Yh - 1][hc], F[0][Yh + 1][hc], F[0][Yh + 2][hc], cy);
-        S.g[e][1][hr][hc] = d1(F[1][Yh - 2][hc], F[1][Yh - 1][hc], F[1][Yh + 1][hc], F[1][Yh + 2][hc], cy);
+      aE[0] -= tz; aE[1] = fma(16.0, tz, aE[1]); aE[2] = fma(-30.0, tz, aE[2]); aE[3] = fma(16.0, tz, aE[3]); aE[4] -= tz;
+      if constexpr (FULL) {
+        const double uym2 = F[0][Y - 2][X], uym1 = F[0][Y - 1][X], uyp1 = F[0][Y + 1][X], uyp2 = F[0][Y + 2][X];
+        const double vxm2 = F[1][Y][X - 2], vxm1 = F[1][Y][X - 1], vxp1 = F[1][Y][X + 1], vxp2 = F[1][Y][X + 2];
+        const double u_y = d1(uym2, uym1, uyp1, uyp2, cy), v_x = d1(vxm2, vxm1, vxp1, vxp2, cx);
+        Au[2] = fma(four3, d2(uxm2, uxm1, u, uxp1, uxp2, cxx), d2(uym2, uym1, u, uyp1, uyp2, cyy));
+        Av[2] = fma(four3, d2(vym2, vym1, v, vyp1, vyp2, cyy), d2(vxm2, vxm1, v, vxp1, vxp2, cxx));
+        S.g[e][0][ty][X] = u_y;
+        S.g[e][1][ty][X] = v_y;
+        Aw[2] = d2(wxm2, wxm1, w, wxp1, wxp2, cxx) + d2(wym2, wym1, w, wyp1, wyp2, cyy);
+        const double lapT = d2(F[3][Y][X - 2], F[3][Y][X - 1], T, F[3][Y][X + 1], F[3][Y][X + 2], cxx) +
+                            d2(F[3][Y - 2][X], F[3][Y - 1][X], T, F[3][Y + 1][X], F[3][Y + 2][X], cyy);
+        const double sxy = u_y + v_x;
+        aE[2] += fma(P.cq, lapT, P.inv_Re * fma(sxy, sxy, 2.0 * fma(u_x, u_x, v_y * v_y)));
+        if (tid < 32) {                                          // x halo columns of the exchange buffer
+          const int Yh = hr + kVH;
+          S.g[e][0][hr][hc] = d1(F[0][Yh - 2][hc], F[0][Yh - 1][hc], F[0][Yh + 1][hc], F[0][Yh + 2][hc], cy);
+          S.g[e][1][hr][hc] = d1(F[1][Yh - 2][hc], F[1][Yh - 1][hc], F[1][Yh + 1][hc], F[1][Yh + 2][hc], cy);
+        }
       }
-    }
-    {
+    };
+    if (k + 2 >= z0 && k + 2 < z1) enter(std::true_type{});
+    else enter(std::false_type{});
+    if (k + 1 >= z0 && k + 1 < z1) {
       // ---- x-y mixed terms of plane k+1: d_x of the d_y values published one step ago
       const double (*G)[kVY][kVPX] = S.g[(k + 1 + 8) & 1];
       Au[1] = fma(third, d1(G[1][ty][X - 2], G[1][ty][X - 1], G[1][ty][X + 1], G[1][ty][X + 2], cx), Au[1]);   // + v_xy / 3
@@ -513,24 +522,25 @@ viscous_tgv_kernel(const __grid_constant__ DevParams P, const double *__restrict
     if (k < z0 || !inside) continue;
 
     // ---- plane k is complete: z-direction terms from the register windows
-    const double u = uw[2], v = vw[2], w = ww[2];
-    const double u_z = d1(uw[0], uw[1], uw[3], uw[4], cz);
-    const double v_z = d1(vw[0], vw[1], vw[3], vw[4], cz);
-    const double w_z = d1(ww[0], ww[1], ww[3], ww[4], cz);
-    const double u_zz = d2(uw[0], uw[1], u, uw[3], uw[4], czz);
-    const double v_zz = d2(vw[0], vw[1], v, vw[3], vw[4], czz);
-    const double w_zz = d2(ww[0], ww[1], w, ww[3], ww[4], czz);
-    const double M0 = Au[0] + fma(third, d1(s0w[0], s0w[1], s0w[3], s0w[4], cz), u_zz);          // + w_xz / 3
-    const double M1 = Av[0] + fma(third, d1(s1w[0], s1w[1], s1w[3], s1w[4], cz), v_zz);          // + w_yz / 3
-    const double M2 = Aw[0] + fma(third, d1(s2w[0], s2w[1], s2w[3], s2w[4], cz), four3 * w_zz);  // + (u_xz + v_yz)/3
+    const double u = uw[C], v = vw[C], w = ww[C];
+    const double u_z = d1(uw[M2], uw[M1], uw[P1], uw[P2], cz);
+    const double v_z = d1(vw[M2], vw[M1], vw[P1], vw[P2], cz);
+    const double w_z = d1(ww[M2], ww[M1], ww[P1], ww[P2], cz);
+    const double u_zz = d2(uw[M2], uw[M1], u, uw[P1], uw[P2], czz);
+    const double v_zz = d2(vw[M2], vw[M1], v, vw[P1], vw[P2], czz);
+    const double w_zz = d2(ww[M2], ww[M1], w, ww[P1], ww[P2], czz);
+    const double M0 = Au[0] + fma(third, d1(s0w[M2], s0w[M1], s0w[P1], s0w[P2], cz), u_zz);          // + w_xz / 3
+    const double M1v = Av[0] + fma(third, d1(s1w[M2], s1w[M1], s1w[P1], s1w[P2], cz), v_zz);         // + w_yz / 3
+    const double M2v = Aw[0] + fma(third, d1(s2w[M2], s2w[M1], s2w[P1], s2w[P2], cz), four3 * w_zz); // + (u_xz + v_yz)/3
     // tau_ij d_j u_i = [2 (u_x^2 + v_y^2 + w_z^2) - 2/3 div^2 + s_xy^2 + s_xz^2 + s_yz^2]/Re; the in-plane part is in aE
-    const double div = s2w[2] + w_z;
-    const double sxz = u_z + s0w[2], syz = v_z + s1w[2];
+    const double div = s2w[C] + w_z;
+    const double sxz = u_z + s0w[C], syz = v_z + s1w[C];
     const double phiz = fma(sxz, sxz, fma(syz, syz, fma(2.0 * w_z, w_z, (-2.0 / 3.0) * (div * div))));
-    const double r1 = M0 * P.inv_Re, r2 = M1 * P.inv_Re, r3 = M2 * P.inv_Re;
+    const double r1 = M0 * P.inv_Re, r2 = M1v * P.inv_Re, r3 = M2v * P.inv_Re;
     const double r4 = fma(u, r1, fma(v, r2, w * r3)) + fma(phiz, P.inv_Re, aE[0]);
-    asm volatile("cp.async.wait_all;" ::: "memory");           // R has landed
-    const double rold[4] = {S.r[0][tid], S.r[1][tid], S.r[2][tid], S.r[3][tid]};
+    asm volatile("cp.async.wait_group 1;" ::: "memory");       // R of node k (issued one step ago) has landed
+    const long long at = L.at(i, j, k);
+    const double rold[4] = {S.r[k & 1][0][tid], S.r[k & 1][1][tid], S.r[k & 1][2][tid], S.r[k & 1][3][tid]};
     R[sv + at] = rold[0] + r1;
     R[2 * sv + at] = rold[1] + r2;
     R[3 * sv + at] = rold[2] + r3;
