@@ -153,6 +153,17 @@ int osbli_rk4_step(osbli_handle h, double *d_Q, double *d_Qtmp, double dt, void 
 int osbli_advance_host(osbli_handle h, double *h_Q, double *d_Q, double *d_Qtmp, double dt,
                        int32_t nsteps, void *cuda_stream);
 
+/* The same for a batch of independent states, pipelined: h_Q[b] (b = 0..nbatch-1, HOST pointers, padded layout,
+ * pinned memory for the copies to be asynchronous) are each advanced by nsteps RK3 steps in place.  Three device
+ * states d_Q[0..2] (DEVICE pointers owned by the caller) rotate through host->device copy, compute and
+ * device->host copy on three streams (the caller's stream computes; two internal non-blocking streams copy), so
+ * that in steady state the cost per state is max(copy in, compute, copy out) instead of their sum.  Host
+ * buffers may repeat with period 3 (h_Q[b] == h_Q[b+3]): the copy-in of b+3 is ordered after the copy-out of b.
+ * Returns after everything has completed (the stream is synchronised).  Results are bit-identical to
+ * osbli_advance_host on each state. */
+int osbli_advance_host_batch(osbli_handle h, double *const *h_Q, int32_t nbatch, double *const *d_Q,
+                             double *d_Qtmp, double dt, int32_t nsteps, void *cuda_stream);
+
 /* Number of kernel launches the handle has enqueued so far (host counter; for bench.py). */
 int osbli_launch_count(osbli_handle h, int64_t *out);
 

@@ -22,6 +22,9 @@ struct osbli_ctx {
   bool profiling;
   std::vector<ProfiledLaunch> *prof;   // events around every launch while profiling
   TmapCache tmaps;                     // tensor maps of the states seen by the fast viscous kernel
+  cudaStream_t s_in, s_out;            // copy streams of osbli_advance_host_batch (created on first use)
+  cudaEvent_t ev_h2d[3], ev_cmp[3], ev_d2h[3];
+  bool pipe_ready;
 };
 
 namespace {
@@ -316,6 +319,56 @@ int osbli_advance_host(osbli_handle h, double *h_Q, double *d_Q, double *d_Qtmp,
   return OSBLI_OK;
 }
 
+static int pipe_setup(osbli_ctx *h) {
+  if (h->pipe_ready) return OSBLI_OK;
+  if (cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking) != cudaSuccess) return OSBLI_ECUDA;
+  if (cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking) != cudaSuccess) return OSBLI_ECUDA;
+  for (int s = 0; s < 3; ++s)
+    if (cudaEventCreateWithFlags(&h->ev_h2d[s], cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_cmp[s], cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_d2h[s], cudaEventDisableTiming) != cudaSuccess)
+      return OSBLI_ECUDA;
+  h->pipe_ready = true;
+  return OSBLI_OK;
+}
+
+int osbli_advance_host_batch(osbli_handle h, double *const *h_Q, int32_t nbatch, double *const *d_Q,
+                             double *d_Qtmp, double dt, int32_t nsteps, void *cuda_stream) {
+  if (!h || !h_Q || !d_Q || !d_Qtmp || nbatch < 0 || nsteps < 0) return OSBLI_EINVAL;
+  for (int s = 0; s < 3; ++s) {
+    if (!d_Q[s] || d_Q[s] == d_Qtmp) return OSBLI_EINVAL;
+    for (int t = 0; t < s; ++t)
+      if (d_Q[s] == d_Q[t]) return OSBLI_EINVAL;
+  }
+  for (int b = 0; b < nbatch; ++b)
+    if (!h_Q[b]) return OSBLI_EINVAL;
+  if (int rc = pipe_setup(h)) return rc;
+  cudaStream_t st = as_stream(cuda_stream);
+  const Layout &L = h->P.L;
+  // work already queued on the caller's stream (it may still use d_Q / d_Qtmp) comes first
+  if (cudaEventRecord(h->ev_cmp[0], st) != cudaSuccess) return OSBLI_ECUDA;
+  if (cudaStreamWaitEvent(h->s_in, h->ev_cmp[0], 0) != cudaSuccess) return OSBLI_ECUDA;
+  for (int b = 0; b < nbatch; ++b) {
+    const int s = b % 3;
+    if (b >= 3 && cudaStreamWaitEvent(h->s_in, h->ev_d2h[s], 0) != cudaSuccess) return OSBLI_ECUDA;   // slot s (and h_Q[b-3]) are free
+    if (copy_interior(L, d_Q[s], h_Q[b], cudaMemcpyHostToDevice, h->s_in) != cudaSuccess) return OSBLI_ECUDA;
+    if (cudaEventRecord(h->ev_h2d[s], h->s_in) != cudaSuccess) return OSBLI_ECUDA;
+    if (cudaStreamWaitEvent(st, h->ev_h2d[s], 0) != cudaSuccess) return OSBLI_ECUDA;
+    if (nsteps == 0)
+      if (int rc = do_bc(h, d_Q[s], st)) return rc;
+    for (int k = 0; k < nsteps; ++k)
+      if (int rc = do_step(h, 3, d_Q[s], d_Qtmp, dt, st)) return rc;
+    if (cudaEventRecord(h->ev_cmp[s], st) != cudaSuccess) return OSBLI_ECUDA;
+    if (cudaStreamWaitEvent(h->s_out, h->ev_cmp[s], 0) != cudaSuccess) return OSBLI_ECUDA;
+    if (copy_interior(L, h_Q[b], d_Q[s], cudaMemcpyDeviceToHost, h->s_out) != cudaSuccess) return OSBLI_ECUDA;
+    if (cudaEventRecord(h->ev_d2h[s], h->s_out) != cudaSuccess) return OSBLI_ECUDA;
+  }
+  for (int s = 0; s < 3 && s < nbatch; ++s)
+    if (cudaStreamWaitEvent(st, h->ev_d2h[s], 0) != cudaSuccess) return OSBLI_ECUDA;   // the caller's stream ends after the last copy-out
+  if (cudaStreamSynchronize(st) != cudaSuccess) return OSBLI_ECUDA;
+  return OSBLI_OK;
+}
+
 int osbli_launch_count(osbli_handle h, int64_t *out) {
   if (!h || !out) return OSBLI_EINVAL;
   *out = h->launches;
@@ -357,6 +410,11 @@ int osbli_destroy(osbli_handle h) {
   if (h->prof) {
     for (ProfiledLaunch &pl : *h->prof) { cudaEventDestroy(pl.t0); cudaEventDestroy(pl.t1); }
     delete h->prof;
+  }
+  if (h->pipe_ready) {
+    cudaStreamDestroy(h->s_in);
+    cudaStreamDestroy(h->s_out);
+    for (int s = 0; s < 3; ++s) { cudaEventDestroy(h->ev_h2d[s]); cudaEventDestroy(h->ev_cmp[s]); cudaEventDestroy(h->ev_d2h[s]); }
   }
   delete h;
   return OSBLI_OK;

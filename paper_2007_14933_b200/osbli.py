@@ -79,6 +79,8 @@ _lib.osbli_rk4_step.restype = C.c_int
 _lib.osbli_rk4_step.argtypes = [_h, _dp, _dp, C.c_double, _dp]
 _lib.osbli_advance_host.restype = C.c_int
 _lib.osbli_advance_host.argtypes = [_h, _dp, _dp, _dp, C.c_double, C.c_int32, _dp]
+_lib.osbli_advance_host_batch.restype = C.c_int
+_lib.osbli_advance_host_batch.argtypes = [_h, C.POINTER(_dp), C.c_int32, C.POINTER(_dp), _dp, C.c_double, C.c_int32, _dp]
 _lib.osbli_launch_count.restype = C.c_int
 _lib.osbli_launch_count.argtypes = [_h, C.POINTER(C.c_int64)]
 _lib.osbli_profile_begin.restype = C.c_int
@@ -93,7 +95,7 @@ _lib.osbli_strerror.restype = C.c_char_p
 _lib.osbli_strerror.argtypes = [C.c_int]
 
 EXPORTS = ("osbli_get_layout", "osbli_workspace_bytes", "osbli_init", "osbli_bc", "osbli_rhs",
-           "osbli_rk3_step", "osbli_rk4_step", "osbli_advance_host", "osbli_launch_count", "osbli_profile_begin", "osbli_profile_end",
+           "osbli_rk3_step", "osbli_rk4_step", "osbli_advance_host", "osbli_advance_host_batch", "osbli_launch_count", "osbli_profile_begin", "osbli_profile_end",
            "osbli_measure_fp64_peak", "osbli_destroy", "osbli_strerror")
 K_CLASSES = ("bc", "primitives", "sweep_x", "sweep_y", "sweep_z", "viscous", "rk_update")
 
@@ -151,6 +153,14 @@ def osbli_rk4_step(handle, q_ptr, qtmp_ptr, dt, stream=0):
 def osbli_advance_host(handle, hq_ptr, q_ptr, qtmp_ptr, dt, nsteps, stream=0):
     _check(_lib.osbli_advance_host(handle, hq_ptr, q_ptr, qtmp_ptr, float(dt), int(nsteps), stream),
            "osbli_advance_host")
+
+
+def osbli_advance_host_batch(handle, hq_ptrs, q_ptrs, qtmp_ptr, dt, nsteps, stream=0):
+    assert len(q_ptrs) == 3
+    hq = (_dp * len(hq_ptrs))(*hq_ptrs)
+    dq = (_dp * 3)(*q_ptrs)
+    _check(_lib.osbli_advance_host_batch(handle, hq, len(hq_ptrs), dq, qtmp_ptr, float(dt), int(nsteps), stream),
+           "osbli_advance_host_batch")
 
 
 def osbli_launch_count(handle) -> int:
@@ -287,6 +297,11 @@ class Solver:
     def advance_host(self, hQ, Q, Qtmp, dt, nsteps):
         osbli_advance_host(self.handle, hQ.data_ptr(), Q.data_ptr(), Qtmp.data_ptr(), dt, nsteps, self._stream())
         return hQ
+
+    def advance_host_batch(self, hQs, Qs, Qtmp, dt, nsteps):
+        osbli_advance_host_batch(self.handle, [t.data_ptr() for t in hQs], [t.data_ptr() for t in Qs], Qtmp.data_ptr(),
+                                 dt, nsteps, self._stream())
+        return hQs
 
     def profile_begin(self):
         osbli_profile_begin(self.handle)

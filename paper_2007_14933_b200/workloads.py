@@ -410,3 +410,29 @@ def perturb(case, seed=0, amp=0.02):
         scale = amp * (0.1 * ref if c in (0, 4) else max(ref, 0.1))
         Q[c][core] += scale * rng.uniform(-1.0, 1.0, size=Q[c][core].shape)
     return edge_pad_interior(Q, case.n)
+
+
+def approximate_metrics(case):
+    """Metric fields D = (dx/dxi)^-1, detJ, E = d(D) of a curvilinear case from 2nd-order numpy gradients of its
+    analytic coordinates.  INPUT GENERATION for throughput runs and memory checks only (bench.py, tests/
+    sanitizer_cases.py), where the values merely have to be smooth, finite and consistent; the parity tests feed
+    both sides the metric fields of PAPER.md:228 computed by the oracle's `metrics_from_coords`."""
+    X = case.coords
+    A = np.zeros((3, 3) + X.shape[1:])
+    axes = {0: 2, 1: 1, 2: 0}
+    for c in range(3):
+        for d in range(3):
+            if case.n[d] > 1:
+                A[c, d] = np.gradient(X[c], axis=axes[d])
+            else:
+                A[c, d] = case.delta[d] if c == d else 0.0
+    Am = np.moveaxis(A, (0, 1), (-2, -1))
+    det = np.linalg.det(Am)
+    D = np.moveaxis(np.linalg.inv(Am), (-2, -1), (0, 1))          # D[k][j] = d xi_k / d x_j
+    IJ = ((0, 0), (0, 1), (0, 2), (1, 1), (1, 2), (2, 2))
+    E = [[None] * 6 for _ in range(3)]
+    for l in range(3):
+        grads = [[np.gradient(D[l, j], axis=axes[k]) if case.n[k] > 1 else 0.0 * det for k in range(3)] for j in range(3)]
+        for m, (i, j) in enumerate(IJ):
+            E[l][m] = np.ascontiguousarray(sum(D[k, i] * grads[j][k] for k in range(3)))
+    return {"D": [[np.ascontiguousarray(D[k, j]) for j in range(3)] for k in range(3)], "detJ": np.ascontiguousarray(det), "E": E}

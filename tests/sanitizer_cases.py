@@ -39,22 +39,6 @@ def periodic_box(n, scheme=W.TENO5, visc=W.VISC_CONST):
     return c
 
 
-def metrics_on_device_free(case):
-    """Metric fields without the oracle: 2nd-order numpy gradients of the analytic coordinates are good enough for
-    a memory check (values only need to be finite and the Jacobian positive)."""
-    X = case.coords
-    A = np.zeros((3, 3) + X.shape[1:])
-    for c in range(3):
-        for d, ax in ((0, 2), (1, 1), (2, 0)):
-            A[c, d] = np.gradient(X[c], axis=ax) if X.shape[1 + ax] > 1 else (1.0 if c == d else 0.0)
-    Am = np.moveaxis(A, (0, 1), (-2, -1))
-    det = np.linalg.det(Am)
-    inv = np.moveaxis(np.linalg.inv(Am), (-2, -1), (0, 1))
-    zero = np.zeros_like(det)
-    return {"D": [[np.ascontiguousarray(inv[k, j]) for j in range(3)] for k in range(3)], "detJ": np.ascontiguousarray(det),
-            "E": [[zero + 1e-3 * (l + m) for m in range(6)] for l in range(3)]}
-
-
 def run(name, case, nsteps, metrics=None, rk4=False):
     sol = osbli.Solver(metrics=metrics, **case.physics())
     Q = sol.to_padded(case.Q0)
@@ -84,7 +68,7 @@ def main():
     run("tgv16_central4", W.tgv(16, scheme=W.CENTRAL4), 2)
     run("tgv16_rk4", W.tgv(16), 1, rk4=True)
     wb = W.wavy_box(n=(40, 21, 9))
-    run("wavy_box (curvilinear, wall / Dirichlet / extrapolation / periodic, Sutherland)", wb, 2, metrics=metrics_on_device_free(wb))
+    run("wavy_box (curvilinear, wall / Dirichlet / extrapolation / periodic, Sutherland)", wb, 2, metrics=W.approximate_metrics(wb))
     ch = W.channel(n=(24, 33, 6), noise=1e-3, scheme=W.TENO5)
     run("channel3d (adiabatic wall, body force)", ch, 2)
     ssp = W.tgv(16)

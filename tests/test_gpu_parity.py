@@ -314,6 +314,32 @@ def test_advance_host_matches_device_steps():
     sol.close()
 
 
+def test_advance_host_batch_pipeline_matches_serial():
+    """osbli_advance_host_batch (three device states, copies and compute on three streams) gives, bit for bit, what
+    osbli_advance_host gives item by item -- including when host buffers repeat with period 3."""
+    torch = _torch()
+    case = W.tgv(32)
+    sol = parity.make_solver(case)
+    inputs = [case.Q0] + [W.perturb(case, seed=s, amp=0.01) for s in (1, 2, 3, 4)]
+    Q, Qtmp = sol.empty_state(), sol.empty_state()
+    ref = []
+    for q0 in inputs:
+        hq = sol.to_padded(q0, pinned_host=True)
+        sol.advance_host(hq, Q, Qtmp, case.dt, 2)
+        ref.append(sol.from_padded(hq))
+    hqs = [sol.to_padded(q0, pinned_host=True) for q0 in inputs]
+    Qs = [sol.empty_state(), sol.empty_state(), sol.empty_state()]
+    sol.advance_host_batch(hqs, Qs, Qtmp, case.dt, 2)
+    for a, b in zip(hqs, ref):
+        assert np.array_equal(parity.interior(case, sol.from_padded(a)), parity.interior(case, b))
+    # period-3 reuse of host buffers: 6 items over 3 buffers = each buffer advanced twice by 1 step = 2 steps
+    hq3 = [sol.to_padded(q0, pinned_host=True) for q0 in inputs[:3]]
+    sol.advance_host_batch([hq3[b % 3] for b in range(6)], Qs, Qtmp, case.dt, 1)
+    for a, b in zip(hq3, ref[:3]):
+        assert np.array_equal(parity.interior(case, sol.from_padded(a)), parity.interior(case, b))
+    sol.close()
+
+
 # ------------------------------------------------- full size, bench launch configuration ----
 def sampled_full_size(name, n, nsamples, presteps):
     """At BASELINE.json's full sizes the oracle is evaluated one node at a time on sampled nodes
