@@ -407,6 +407,18 @@ def run_ours(args):
         "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peak_src,
     }
 
+    if case.scheme == W.CENTRAL4 and prof["sweep_x"][1] == 0 and prof["viscous"][1] == 0:
+        # fused central path (osbli_central.cu): one kernel per stage, bound by HBM.  Algorithmic bytes per point:
+        # Q in + dU out + Qout out = 120 in the first stage (dU is not read), 160 in the others.
+        zms, zcnt = prof["sweep_z"]
+        avg_s = zms * 1e-3 / max(zcnt, 1)
+        bytes_point = (120 + 160 + 160) / 3.0
+        gbs = bytes_point * npts / avg_s * 1e-9
+        roofline.update({"bound": "hbm", "kernel": "central_fused", "achieved": gbs, "peak": peaks.get("hbm_gbs"), "unit": "GB/s",
+                         "frac": gbs / peaks.get("hbm_gbs"), "algorithmic_bytes_per_point": bytes_point, "avg_launch_ms": avg_s * 1e3,
+                         "peak_source": peak_src, "traffic": None, "traffic_source": None,
+                         "fp64_useful_tflops": step_flop * value / world * 1e-12})
+
     # the oracle beside it: all cores on a bounded sample of the same workload, and one core on a small one
     cpu_case, cpu_what = cpu_sample_case(args, full=True)
     cpu_rate, cpu_cores, cpu_dt = cpu_oracle_rate(cpu_case)

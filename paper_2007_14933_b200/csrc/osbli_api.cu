@@ -158,6 +158,21 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
 // so the state moves Q -> Q2 -> Q3 (-> Q2 -> Q3) -> Q through two workspace states; 1-D problems use the
 // separate in-place update kernel.  The result is in Q either way.
 int do_step(osbli_ctx *h, int nstages, double *Q, double *Qtmp, double dt, cudaStream_t st) {
+  if (central_fused_path(h->P)) {
+    // central scheme on a uniform triply periodic grid: one kernel per stage (convective + viscous terms, stage
+    // update, periodic images of the new state), Q -> Q2 -> Q3 (-> Q2 -> Q3) -> Q; one halo fill per step
+    for (int s = 0; s < nstages; ++s) {
+      double *src = s == 0 ? Q : ((s & 1) ? h->Q2 : h->Q3);
+      double *dst = s == nstages - 1 ? Q : ((s & 1) ? h->Q3 : h->Q2);
+      if (s == 0)
+        if (int rc = do_bc(h, src, st)) return rc;
+      RkArgs rk;
+      rk_coefficients(nstages, h->P.rk3_form, s, &rk.A, &rk.B);
+      rk.dt = dt; rk.Qtmp = Qtmp; rk.Qout = dst; rk.first = (rk.A == 0.0); rk.wrap = 1;
+      OSBLI_LAUNCH(h, OSBLI_K_SWEEP_Z, st, launch_central_fused(h->P, src, rk, &h->tmaps, st));
+    }
+    return OSBLI_OK;
+  }
   const bool fuse = (h->P.L.n[1] > 1 || h->P.L.n[2] > 1) && h->P.scheme != OSBLI_SCHEME_CENTRAL4;
   bool wrap = fuse;                  // every active direction periodic: the fused update fills the halos itself
   for (int d = 0; d < 3; ++d)
@@ -220,7 +235,7 @@ int osbli_init(const osbli_params *p, void *d_workspace, size_t workspace_bytes,
   if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return OSBLI_ECUDA;
   if (prop.major != 10) return OSBLI_ECUDA;                      // sm_100a code only; no other path exists
   // opt-in shared-memory sizes are per device: set them for the device this handle lives on
-  if (sweep_set_attributes() != cudaSuccess || viscous_set_attributes() != cudaSuccess) return OSBLI_ECUDA;
+  if (sweep_set_attributes() != cudaSuccess || viscous_set_attributes() != cudaSuccess || central_set_attributes() != cudaSuccess) return OSBLI_ECUDA;
 
   osbli_ctx *h = new (std::nothrow) osbli_ctx;
   if (!h) return OSBLI_EINVAL;

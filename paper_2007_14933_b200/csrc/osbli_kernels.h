@@ -34,6 +34,12 @@ cudaError_t launch_viscous_fast(const DevParams &P, const double *Q, double *R, 
 cudaError_t sweep_set_attributes();
 cudaError_t viscous_set_attributes();
 
+// scheme 4 on uniform triply periodic grids with mu = 1 (osbli_central.cu): convective + viscous terms + stage update
+// + periodic write-through in one kernel per stage; Q -> rk.Qout, dU = rk.Qtmp in place
+bool central_fused_path(const DevParams &P);
+cudaError_t central_set_attributes();
+cudaError_t launch_central_fused(const DevParams &P, const double *Q, const RkArgs &rk, TmapCache *cache, cudaStream_t st);
+
 // central convective terms, scheme 4 (osbli_visc.cu): R = - sum_d delta_d F_d on interior nodes (writes R)
 cudaError_t launch_central(const DevParams &P, const double *Q, double *R, cudaStream_t st);
 

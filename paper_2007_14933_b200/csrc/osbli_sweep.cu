@@ -25,27 +25,6 @@ namespace osbli {
 #ifndef OSBLI_X_MINB
 #define OSBLI_X_MINB 1
 #endif
-// Periodic images of one node of the fused update (rare path, kept out of line so that it costs the
-// marching loop no registers).  mask: bits 0/1 = x image at +nx / -nx, bits 2/3 = transverse, bits
-// 4/5 = sweep direction; ox, ot, os = the three image offsets in doubles.
-__device__ __noinline__ void wrap_store(double *dst, long long sv, int mask, long long ox, long long ot, long long os,
-                                        double q0, double q1, double q2, double q3, double q4) {
-  const int xm = mask & 3, tm = (mask >> 2) & 3, sm = mask >> 4;
-  for (int a = 0; a < 3; ++a) {
-    if (a && !(sm & a)) continue;
-    for (int b = 0; b < 3; ++b) {
-      if (b && !(tm & b)) continue;
-      for (int e = 0; e < 3; ++e) {
-        if (e && !(xm & e)) continue;
-        if (!(a | b | e)) continue;
-        double *p = dst + (a == 1 ? os : (a == 2 ? -os : 0)) + (b == 1 ? ot : (b == 2 ? -ot : 0)) +
-                    (e == 1 ? ox : (e == 2 ? -ox : 0));
-        p[0] = q0; p[sv] = q1; p[2 * sv] = q2; p[3 * sv] = q3; p[4 * sv] = q4;
-      }
-    }
-  }
-}
-
 // RK = 0: R (-)= flux difference.  RK = 1 / 2: this is the last kernel of the stage and also does
 // the low-storage Runge-Kutta update eq. (36)-(37) of its nodes (1: first stage, A_0 = 0, dU is not
 // read): with R_in the residual accumulated by the earlier kernels of the stage,
