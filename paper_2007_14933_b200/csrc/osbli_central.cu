@@ -25,34 +25,43 @@
 
 namespace osbli {
 
+#ifndef OSBLI_CCHUNK
+#define OSBLI_CCHUNK 64
+#endif
+#ifndef OSBLI_CY
+#define OSBLI_CY 8
+#endif
+constexpr int kCY = OSBLI_CY, kCPY = kCY + 2 * kVH;              // tile rows of this kernel: 32 x kCY nodes, 36 x (kCY + 4) staged
+constexpr unsigned kCTileBytes = 5 * kCPY * kVPX * sizeof(double);
+
 struct CSmem {
-  double tile[2][5][kVPY][kVPX];       // TMA destinations (128-byte aligned: first member), double buffered
-  double f[2][6][kVPY][kVPX];          // u, v, w, T, rho, G: the plane being staged and the plane entering
-  double g[2][2][kVY][kVPX];           // d_y u, d_y v of the tile rows incl. the x halo, double buffered
-  double q[2][10][kVX * kVY];          // per-thread slots: Q (0-4) and dU (5-9) of the two nodes in flight
-  unsigned long long mbar[2];
+  double tile[3][5][kCPY][kVPX];       // TMA destinations (128-byte aligned: first member), fetched two planes ahead
+  double f[2][6][kCPY][kVPX];          // u, v, w, T, rho, G: the plane being staged and the plane entering
+  double g[2][2][kCY][kVPX];           // d_y u, d_y v of the tile rows incl. the x halo, double buffered
+  double q[2][10][kVX * kCY];          // per-thread slots: Q (0-4) and dU (5-9) of the two nodes in flight
+  unsigned long long mbar[3];
 };
 
 template <bool FIRST>
-__global__ void __launch_bounds__(kVX * kVY, 1)
+__global__ void __launch_bounds__(kVX * kCY, 1)
 central_fused_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, int chunk,
                      const __grid_constant__ CUtensorMap tmap, const RkArgs rk) {
   extern __shared__ __align__(128) unsigned char cs_raw[];
   CSmem &S = *reinterpret_cast<CSmem *>(cs_raw);
   const Layout &L = P.L;
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * kVX + tx;
-  const int x0 = blockIdx.x * kVX, y0 = blockIdx.y * kVY;
+  const int x0 = blockIdx.x * kVX, y0 = blockIdx.y * kCY;
   const int z0 = blockIdx.z * chunk, z1 = min(z0 + chunk, L.n[2]);
   const int i = x0 + tx, j = y0 + ty;
   const bool inside = i < L.n[0] && j < L.n[1];
   const long long sv = L.sv;
 
-  constexpr int NPT = kVPX * kVPY;                                // 432 tile points, up to two per thread
+  constexpr int NPT = kVPX * kCPY;                                // 432 tile points, up to two per thread
   int pi[2], pj[2];
   bool pv[2];
 #pragma unroll
   for (int s = 0; s < 2; ++s) {
-    const int t = tid + s * (kVX * kVY);
+    const int t = tid + s * (kVX * kCY);
     pv[s] = t < NPT;
     const int yy = pv[s] ? t / kVPX : 0, xx = pv[s] ? t % kVPX : 0;
     pi[s] = xx; pj[s] = yy;
@@ -60,15 +69,15 @@ central_fused_kernel(const __grid_constant__ DevParams P, const double *__restri
   }
   auto fetch = [&](int plane) {
     if (tid == 0) {
-      const int b = (plane - (z0 - 2)) & 1;
-      mbar_expect_tx(&S.mbar[b], kVTileBytes);
+      const int b = (plane - (z0 - 2)) % 3;
+      mbar_expect_tx(&S.mbar[b], kCTileBytes);
       tma_load_4d(&S.tile[b][0][0][0], &tmap, (int)L.xoff + x0 - kVH, L.h[1] + y0 - kVH, L.h[2] + plane, 0, &S.mbar[b]);
     }
   };
   auto stage = [&](int plane) {
     const int slot = (plane + 8) & 1;
-    const int jj = plane - (z0 - 2), b = jj & 1;
-    mbar_wait(&S.mbar[b], (unsigned)(jj >> 1) & 1u);
+    const int jj = plane - (z0 - 2), b = jj % 3;               // the mbarrier of buffer b has completed jj / 3 phases before
+    mbar_wait(&S.mbar[b], (unsigned)(jj / 3) & 1u);
 #pragma unroll
     for (int s = 0; s < 2; ++s)
       if (pv[s]) {
@@ -88,6 +97,7 @@ central_fused_kernel(const __grid_constant__ DevParams P, const double *__restri
   if (tid == 0) {
     mbar_init(&S.mbar[0], 1);
     mbar_init(&S.mbar[1], 1);
+    mbar_init(&S.mbar[2], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -117,6 +127,7 @@ central_fused_kernel(const __grid_constant__ DevParams P, const double *__restri
   fetch(z0 - 2);
   stage(z0 - 2);
   fetch(z0 - 1);
+  fetch(z0);
   __syncthreads();
   const int X = tx + kVH, Y = ty + kVH;
   const int hr = tid >> 2, hc = (tid & 3) < 2 ? (tid & 3) : kVX + (tid & 3);
@@ -158,7 +169,7 @@ central_fused_kernel(const __grid_constant__ DevParams P, const double *__restri
       }
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
-    if (k + 4 < z1 + 2) fetch(k + 4);
+    if (k + 5 < z1 + 2) fetch(k + 5);                          // raw plane k+5 into the buffer plane k+2 has left
 #pragma unroll
     for (int m = 0; m < 4; ++m) {
       uw[m] = uw[m + 1]; vw[m] = vw[m + 1]; ww[m] = ww[m + 1]; rw[m] = rw[m + 1]; Gw[m] = Gw[m + 1]; pw[m] = pw[m + 1];
@@ -171,7 +182,7 @@ central_fused_kernel(const __grid_constant__ DevParams P, const double *__restri
     auto enter = [&](auto full_tag) {
       constexpr bool FULL = decltype(full_tag)::value;
       const int e = (k + 2 + 8) & 1;
-      const double (*F)[kVPY][kVPX] = S.f[e];
+      const double (*F)[kCPY][kVPX] = S.f[e];
       const double u = F[0][Y][X], v = F[1][Y][X], w = F[2][Y][X], T = F[3][Y][X], r = F[4][Y][X], G = F[5][Y][X];
       const double ux[4] = {F[0][Y][X - 2], F[0][Y][X - 1], F[0][Y][X + 1], F[0][Y][X + 2]};
       const double vy[4] = {F[1][Y - 2][X], F[1][Y - 1][X], F[1][Y + 1][X], F[1][Y + 2][X]};
@@ -216,7 +227,7 @@ central_fused_kernel(const __grid_constant__ DevParams P, const double *__restri
         }
         B0[2] = -cv[0]; B1[2] = Au - cv[1]; B2[2] = Av - cv[2]; B3[2] = Aw - cv[3];
         aE[2] += ev - cv[4];
-        if (tid < 32) {                                          // x halo columns of the exchange buffer
+        if (tid < 4 * kCY) {                                     // x halo columns of the exchange buffer
           const int Yh = hr + kVH;
           S.g[e][0][hr][hc] = d1(F[0][Yh - 2][hc], F[0][Yh - 1][hc], F[0][Yh + 1][hc], F[0][Yh + 2][hc], cy);
           S.g[e][1][hr][hc] = d1(F[1][Yh - 2][hc], F[1][Yh - 1][hc], F[1][Yh + 1][hc], F[1][Yh + 2][hc], cy);
@@ -227,7 +238,7 @@ central_fused_kernel(const __grid_constant__ DevParams P, const double *__restri
     else enter(std::false_type{});
     if (k + 1 >= z0 && k + 1 < z1) {
       // ---- x-y mixed terms of plane k+1 (d_x of the d_y values published one step ago), divided by 3 Re
-      const double (*Gm)[kVY][kVPX] = S.g[(k + 1 + 8) & 1];
+      const double (*Gm)[kCY][kVPX] = S.g[(k + 1 + 8) & 1];
       const double vxy = (third * P.inv_Re) * d1(Gm[1][ty][X - 2], Gm[1][ty][X - 1], Gm[1][ty][X + 1], Gm[1][ty][X + 2], cx);
       const double uxy = (third * P.inv_Re) * d1(Gm[0][ty][X - 2], Gm[0][ty][X - 1], Gm[0][ty][X + 1], Gm[0][ty][X + 2], cx);
       B1[1] += vxy;
@@ -284,12 +295,13 @@ cudaError_t central_set_attributes() {
 
 cudaError_t launch_central_fused(const DevParams &P, const double *Q, const RkArgs &rk, TmapCache *cache, cudaStream_t st) {
   const Layout &L = P.L;
-  const int chunk = L.n[2] > 32 ? 32 : L.n[2];
-  dim3 grid((L.n[0] + kVX - 1) / kVX, (L.n[1] + kVY - 1) / kVY, (L.n[2] + chunk - 1) / chunk);
-  const CUtensorMap *map = state_tensor_map(L, Q, cache);
+  // 64 planes per block: 6 warm-up planes per chunk (9 %); at 256^3 1024 blocks = 6.9 waves of one block per SM
+  const int chunk = L.n[2] > OSBLI_CCHUNK ? OSBLI_CCHUNK : L.n[2];
+  dim3 grid((L.n[0] + kVX - 1) / kVX, (L.n[1] + kCY - 1) / kCY, (L.n[2] + chunk - 1) / chunk);
+  const CUtensorMap *map = state_tensor_map(L, Q, cache, kCPY);
   if (!map) return cudaErrorNotSupported;
-  if (rk.first) central_fused_kernel<true><<<grid, dim3(kVX, kVY), sizeof(CSmem), st>>>(P, Q, chunk, *map, rk);
-  else central_fused_kernel<false><<<grid, dim3(kVX, kVY), sizeof(CSmem), st>>>(P, Q, chunk, *map, rk);
+  if (rk.first) central_fused_kernel<true><<<grid, dim3(kVX, kCY), sizeof(CSmem), st>>>(P, Q, chunk, *map, rk);
+  else central_fused_kernel<false><<<grid, dim3(kVX, kCY), sizeof(CSmem), st>>>(P, Q, chunk, *map, rk);
   return cudaGetLastError();
 }
 

@@ -23,9 +23,10 @@ cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *pr
 // fused fast path (uniform grid, mu = 1, three periodic directions): reads Q directly, R += viscous terms
 bool viscous_fast_path(const DevParams &P);
 struct TmapCache {                    // tensor maps of the states the fast viscous kernel has been launched on (host side)
-  static constexpr int kSlots = 4;
+  static constexpr int kSlots = 6;
   struct alignas(64) Map { unsigned long long opaque[16]; } map[kSlots];   // CUtensorMap (128 bytes, 64-byte aligned)
   const double *ptr[kSlots];
+  int rows[kSlots];                   // box height the map was encoded for
   int count, next;
 };
 cudaError_t launch_viscous_fast(const DevParams &P, const double *Q, double *R, TmapCache *cache, cudaStream_t st);

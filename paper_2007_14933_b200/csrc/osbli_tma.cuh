@@ -42,7 +42,7 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, i
 // 4-D tensor map over a state: (x incl. row padding, y incl. halo, z incl. halo, variable), box = one plane
 // tile of all five variables.  The encoder lives in the driver library; it is fetched through the runtime
 // so that libosbli links against nothing but cudart.
-inline bool encode_state_map(const Layout &L, const double *Q, CUtensorMap *map) {
+inline bool encode_state_map(const Layout &L, const double *Q, CUtensorMap *map, int box_rows = kVPY) {
   typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                 const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                 CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -59,7 +59,7 @@ inline bool encode_state_map(const Layout &L, const double *Q, CUtensorMap *map)
   if (!fn) return false;
   const cuuint64_t dims[4] = {(cuuint64_t)L.sy, (cuuint64_t)(L.n[1] + 2 * L.h[1]), (cuuint64_t)(L.n[2] + 2 * L.h[2]), 5};
   const cuuint64_t strides[3] = {(cuuint64_t)L.sy * 8, (cuuint64_t)L.sz * 8, (cuuint64_t)L.sv * 8};
-  const cuuint32_t box[4] = {kVPX, kVPY, 1, 5};
+  const cuuint32_t box[4] = {kVPX, (cuuint32_t)box_rows, 1, 5};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double *>(Q), dims, strides, box, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -68,15 +68,16 @@ inline bool encode_state_map(const Layout &L, const double *Q, CUtensorMap *map)
 
 // The tensor map depends on the state's base address only; a step cycles through three states (Q, Q2, Q3), so
 // the handle keeps a small cache and the driver's encoder runs once per address instead of once per launch.
-inline const CUtensorMap *state_tensor_map(const Layout &L, const double *Q, TmapCache *cache) {
+inline const CUtensorMap *state_tensor_map(const Layout &L, const double *Q, TmapCache *cache, int box_rows = kVPY) {
   static_assert(sizeof(CUtensorMap) == sizeof(cache->map[0]), "TmapCache::map must hold a CUtensorMap");
   int hit = -1;
   for (int e = 0; e < cache->count; ++e)
-    if (cache->ptr[e] == Q) hit = e;
+    if (cache->ptr[e] == Q && cache->rows[e] == box_rows) hit = e;
   if (hit < 0) {
     hit = cache->count < TmapCache::kSlots ? cache->count++ : (cache->next++ % TmapCache::kSlots);
-    if (!encode_state_map(L, Q, reinterpret_cast<CUtensorMap *>(&cache->map[hit]))) { cache->count = 0; return nullptr; }
+    if (!encode_state_map(L, Q, reinterpret_cast<CUtensorMap *>(&cache->map[hit]), box_rows)) { cache->count = 0; return nullptr; }
     cache->ptr[hit] = Q;
+    cache->rows[hit] = box_rows;
   }
   return reinterpret_cast<const CUtensorMap *>(&cache->map[hit]);
 }
