@@ -84,6 +84,11 @@ def main():
     ap.add_argument("--threads", type=int, default=os.cpu_count() or 1)
     ap.add_argument("--steps", type=int, default=None, help="debug: stop after this many steps (file marked partial)")
     ap.add_argument("--out", type=str, default=str(GOLDEN))
+    ap.add_argument("--resume-dir", type=str, default=None,
+                    help="directory for restart files (the state every --resume-every steps); an interrupted run continues from there")
+    ap.add_argument("--resume-every", type=int, default=5)
+    ap.add_argument("--stop-after-seconds", type=float, default=None,
+                    help="write a restart file and exit (status 3) once this much wall time has passed")
     a = ap.parse_args()
 
     use_private_library()
@@ -100,19 +105,42 @@ def main():
     q0_hash = sample_hash(sample_of(case, case.Q0, stride))
 
     Q = case.Q0.copy()
-    dU = np.zeros_like(Q)
+    dU = np.zeros_like(Q)          # dU^(0) is never read (A_1 = 0): the state Q alone restarts a run exactly
     R = np.zeros_like(Q)
     out = {}
     t0 = time.time()
     step = 0
+    rdir = Path(a.resume_dir) if a.resume_dir else None
+    tag = f"config{a.config}_{src_hash[:12]}_{q0_hash[:12]}"
+
+    def save_restart():
+        rdir.mkdir(parents=True, exist_ok=True)
+        np.save(rdir / f"{tag}_state.tmp.npy", Q)
+        os.replace(rdir / f"{tag}_state.tmp.npy", rdir / f"{tag}_state.npy")
+        np.savez(rdir / f"{tag}_samples.tmp.npz", step=step, **out)
+        os.replace(rdir / f"{tag}_samples.tmp.npz", rdir / f"{tag}_samples.npz")
+
+    if rdir is not None and (rdir / f"{tag}_samples.npz").exists() and (rdir / f"{tag}_state.npy").exists():
+        z = np.load(rdir / f"{tag}_samples.npz")
+        step = int(z["step"])
+        out = {k: z[k] for k in z.files if k != "step"}
+        Q = np.load(rdir / f"{tag}_state.npy")
+        print(f"config {a.config}: resuming at step {step} from {rdir}", flush=True)
     for cp in checkpoints:
         while step < cp:
             orc.rk3_step(Q, dU, R, case.dt)
             step += 1
+            if rdir is not None and (step % a.resume_every == 0 or (a.stop_after_seconds and time.time() - t0 > a.stop_after_seconds)):
+                save_restart()
+                if a.stop_after_seconds and time.time() - t0 > a.stop_after_seconds and step < checkpoints[-1]:
+                    print(f"config {a.config}: stopped at step {step} after {time.time() - t0:.0f} s (restart file written)", flush=True)
+                    sys.exit(3)
             if step % 5 == 0 or step == cp:
                 el = time.time() - t0
                 print(f"config {a.config}: step {step}/{checkpoints[-1]}  {el:8.1f} s  "
                       f"({3 * case.npoints * step / el:.3e} updates/s, {a.threads} threads)", flush=True)
+        if f"state_{cp}" in out:
+            continue                                   # checkpoint already sampled before the restart
         assert np.isfinite(Q).all()
         out[f"state_{cp}"] = sample_of(case, Q, stride)
         qi = orc.interior(Q)
