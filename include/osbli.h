@@ -105,7 +105,8 @@ int osbli_get_layout(const osbli_params *p, osbli_layout *out);
 
 /* Bytes of device workspace osbli_init needs: three states (the residual R and the two
  * intermediate states Q2, Q3 of osbli_rk3_step, see there) and, when visc != NONE, the staged
- * primitive fields u, v, w, T (and mu for Sutherland). */
+ * primitive fields u, v, w, T (and mu for Sutherland) with their first differences along x, y, z
+ * (16 or 20 scalar fields; "store some"). */
 int osbli_workspace_bytes(const osbli_params *p, size_t *out);
 
 /* Validates *p, records it and the workspace (DEVICE pointer, 256-byte aligned, >= the size

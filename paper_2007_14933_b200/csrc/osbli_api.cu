@@ -45,8 +45,15 @@ int make_layout(const osbli_params *p, Layout *L) {
   return OSBLI_OK;
 }
 
+// workspace fields of the general viscous path: staged u, v, w, T (, mu) and their first differences along x, y, z
+// (none on the fast path -- uniform grid, mu = 1, three active periodic directions -- whose kernels read Q directly)
 int nprim(const osbli_params *p) {
-  return p->visc == OSBLI_VISC_NONE ? 0 : (p->visc == OSBLI_VISC_SUTHERLAND ? 5 : 4);
+  if (p->visc == OSBLI_VISC_NONE) return 0;
+  bool fast = !p->metrics && p->visc == OSBLI_VISC_CONST;
+  const int n[3] = {p->nx, p->ny, p->nz};
+  for (int d = 0; d < 3; ++d)
+    if (n[d] <= 1 || p->bc[d][0] != OSBLI_BC_PERIODIC || p->bc[d][1] != OSBLI_BC_PERIODIC) fast = false;
+  return fast ? 0 : 4 * (p->visc == OSBLI_VISC_SUTHERLAND ? 5 : 4);
 }
 
 int validate(const osbli_params *p) {

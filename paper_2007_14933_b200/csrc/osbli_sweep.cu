@@ -340,8 +340,11 @@ template <int SCHEME, bool CURV>
 static cudaError_t launch_x(const DevParams &P, const double *Q, double *R, int accumulate, cudaStream_t st) {
   const int nlines = P.L.n[1] * P.L.n[2];
   const int nx = P.L.n[0];
+  // segments of 64 nodes (6 warm-up nodes each); small problems (config 4: 2000 lines) take shorter segments until
+  // there are at least as many warps as the chip holds resident (148 SMs x 8)
   int chunk = 64;
-  if (nx <= 64) chunk = ((nx + kXT - 1) / kXT) * kXT;
+  while (chunk > 16 && (long long)((nlines + 31) / 32) * ((nx + chunk - 1) / chunk) < 148LL * 8) chunk /= 2;
+  if (nx <= chunk) chunk = ((nx + kXT - 1) / kXT) * kXT;
   dim3 grid((nlines + kXWarps * 32 - 1) / (kXWarps * 32), (nx + chunk - 1) / chunk, 1);
   const size_t smem = sizeof(XSmem<CURV>) * kXWarps;
   sweep_x_kernel<SCHEME, CURV><<<grid, kXWarps * 32, smem, st>>>(P, Q, R, chunk, accumulate);
@@ -358,6 +361,8 @@ static cudaError_t launch_yz(const DevParams &P, const double *Q, double *R, int
   // segments of 64 nodes (6 warm-up nodes each) where that still leaves >= 4 waves of blocks, else 32
   int chunk = n > 64 ? 32 : n;
   if (n > 64 && (long long)((nx + bx - 1) / bx) * nt * ((n + 63) / 64) >= 4LL * 2 * 148) chunk = 64;
+  // small problems: 16-node segments when 32-node ones leave warp slots of the chip (148 SMs x 8 warps) empty
+  if (n > 16 && chunk >= 32 && (long long)((nx + bx - 1) / bx) * (bx / 32) * nt * ((n + chunk - 1) / chunk) < 148LL * 8) chunk = 16;
   dim3 grid((nx + bx - 1) / bx, nt, (n + chunk - 1) / chunk);
   const RkArgs none = {0.0, 0.0, 0.0, nullptr, nullptr, 0, 0};
   if (rk) {

@@ -3,10 +3,14 @@
 // and the one-sided closures of eq. (30)-(35), next to non-periodic boundaries;
 // metric chain rule on curvilinear grids.
 //
-// Two kernels: (1) point-wise u, v, w, T (, mu) staged once per stage on the halo-extended grid
-// (the paper's "store some" idea: keep the few fields every derivative needs,
-// recompute the rest); (2) one thread per node assembling all derivatives from those fields and
-// adding  d_j tau_ij,  d_j(u_i tau_ij) - d_j q_j  to R.
+// General path, three kernels (the paper's "store some" idea: "the derivatives of the velocity
+// components ... are stored ... to be reused in the mixed derivatives", everything else is recomputed):
+// (1) point-wise u, v, w, T (, mu) staged once per stage on the halo-extended grid; (2) their first
+// differences delta_l f along every active direction (closures included), stored where a mixed difference
+// will read them; (3) one thread per node: second differences from the staged fields, mixed differences
+// delta_k(delta_l f) as ONE five-point stencil over the stored first differences (4-5 loads instead of the
+// 16-25 of a nested evaluation: the curvilinear chain rule needs all 12 of them), assembly of
+// d_j tau_ij,  d_j(u_i tau_ij) - d_j q_j  and R +=.
 #include "osbli_kernels.h"
 
 #include "osbli_tma.cuh"
@@ -62,10 +66,42 @@ __device__ __forceinline__ int d2_stencil(int n, int i, int per, double (&c)[5])
   return -2;
 }
 
+// grad[(f * 3 + l) * sv + at] = delta_l f (computational difference incl. the 1/(12 Delta) factor) at every node whose
+// l-index is interior and whose other indices lie in the interior extended by 2 along periodic directions
+// (where the mixed differences of interior nodes reach).
+template <int NF>
+__global__ void __launch_bounds__(128)
+gradients_kernel(const __grid_constant__ DevParams P, const double *__restrict__ prim, double *__restrict__ grad, int curv) {
+  const Layout &L = P.L;
+  int ext[3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) ext[d] = (L.n[d] > 1 && P.periodic[d]) ? 2 : 0;
+  const int nd[3] = {(int)(blockIdx.x * blockDim.x + threadIdx.x) - ext[0], (int)blockIdx.y - ext[1], (int)blockIdx.z - ext[2]};
+  if (nd[0] >= L.n[0] + ext[0]) return;
+  const long long at = L.at(nd[0], nd[1], nd[2]);
+  const long long sv = L.sv;
+  const long long st[3] = {1, L.sy, L.sz};
+#pragma unroll
+  for (int l = 0; l < 3; ++l) {
+    if (L.n[l] <= 1 || nd[l] < 0 || nd[l] >= L.n[l]) continue;
+    double a[5];
+    const int o = d1_stencil(L.n[l], nd[l], P.periodic[l], a);
+    const double sc = curv ? (1.0 / 12.0) : P.inv12d[l];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      double acc = 0.0;
+#pragma unroll
+      for (int m = 0; m < 5; ++m)
+        if (a[m] != 0.0) acc = fma(a[m] * sc, __ldg(prim + f * sv + at + (long long)(o + m) * st[l]), acc);
+      grad[(f * 3 + l) * sv + at] = acc;
+    }
+  }
+}
+
 template <bool CURV, bool SUTH>
 __global__ void __launch_bounds__(128)
-viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ prim, double *__restrict__ R,
-               int accumulate) {
+viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ prim, const double *__restrict__ grad,
+               double *__restrict__ R, int accumulate) {
   const Layout &L = P.L;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= L.n[0]) return;
@@ -88,21 +124,14 @@ viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ p
   }
   auto F = [&](int f, long long off) { return __ldg(prim + f * sv + at + off); };
 
-  // computational differences: c1[f][k] = delta_k f, c2[f][k][l] = delta_kl f
+  // computational differences: c1[f][k] = delta_k f (stored by gradients_kernel), c2[f][k][l] = delta_kl f
   constexpr int NF1 = SUTH ? 5 : 4;
+  auto Gd = [&](int f, int l, long long off) { return __ldg(grad + (f * 3 + l) * sv + at + off); };
   double c1[5][3], c2[4][3][3];
 #pragma unroll
   for (int f = 0; f < 5; ++f)
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
-      double acc = 0.0;
-      if (f < NF1 && act[k]) {
-#pragma unroll
-        for (int m = 0; m < 5; ++m)
-          if (a1[k][m] != 0.0) acc = fma(a1[k][m], F(f, (long long)(o1[k] + m) * st[k]), acc);
-      }
-      c1[f][k] = acc;
-    }
+    for (int k = 0; k < 3; ++k) c1[f][k] = (f < NF1 && act[k]) ? Gd(f, k, 0) : 0.0;
 #pragma unroll
   for (int f = 0; f < 4; ++f)
 #pragma unroll
@@ -117,16 +146,10 @@ viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ p
 #pragma unroll
             for (int m = 0; m < 5; ++m) acc = fma(a2[k][m], F(f, (long long)(o2[k] + m) * st[k]), acc);
           } else {
+            // delta_k (delta_l f), k < l: the first-difference stencil along k over the stored delta_l f
 #pragma unroll
-            for (int a = 0; a < 5; ++a) {
-              if (a1[k][a] == 0.0) continue;
-              double in = 0.0;
-#pragma unroll
-              for (int b = 0; b < 5; ++b)
-                if (a1[l][b] != 0.0)
-                  in = fma(a1[l][b], F(f, (long long)(o1[k] + a) * st[k] + (long long)(o1[l] + b) * st[l]), in);
-              acc = fma(a1[k][a], in, acc);
-            }
+            for (int a = 0; a < 5; ++a)
+              if (a1[k][a] != 0.0) acc = fma(a1[k][a], Gd(f, l, (long long)(o1[k] + a) * st[k]), acc);
           }
         }
         c2[f][k][l] = acc;
@@ -286,13 +309,25 @@ cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *pr
                            cudaStream_t st) {
   (void)Q;
   const Layout &L = P.L;
+  const bool curv = P.curvilinear != 0, suth = P.visc == 2;
+  // stored first differences live behind the staged primitive fields in the workspace (osbli_workspace_bytes)
+  double *grad = const_cast<double *>(prim) + (long long)(suth ? 5 : 4) * L.sv;
+  {
+    int ext[3];
+    for (int d = 0; d < 3; ++d) ext[d] = (L.n[d] > 1 && P.periodic[d]) ? 2 : 0;
+    const int NX = L.n[0] + 2 * ext[0];
+    dim3 grid((NX + 127) / 128, L.n[1] + 2 * ext[1], L.n[2] + 2 * ext[2]);
+    if (suth) gradients_kernel<5><<<grid, 128, 0, st>>>(P, prim, grad, curv ? 1 : 0);
+    else gradients_kernel<4><<<grid, 128, 0, st>>>(P, prim, grad, curv ? 1 : 0);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
   const int bx = L.n[0] >= 128 ? 128 : 64;
   dim3 grid((L.n[0] + bx - 1) / bx, L.n[1], L.n[2]);
-  const bool curv = P.curvilinear != 0, suth = P.visc == 2;
-  if (curv && suth) viscous_kernel<true, true><<<grid, bx, 0, st>>>(P, prim, R, accumulate);
-  else if (curv) viscous_kernel<true, false><<<grid, bx, 0, st>>>(P, prim, R, accumulate);
-  else if (suth) viscous_kernel<false, true><<<grid, bx, 0, st>>>(P, prim, R, accumulate);
-  else viscous_kernel<false, false><<<grid, bx, 0, st>>>(P, prim, R, accumulate);
+  if (curv && suth) viscous_kernel<true, true><<<grid, bx, 0, st>>>(P, prim, grad, R, accumulate);
+  else if (curv) viscous_kernel<true, false><<<grid, bx, 0, st>>>(P, prim, grad, R, accumulate);
+  else if (suth) viscous_kernel<false, true><<<grid, bx, 0, st>>>(P, prim, grad, R, accumulate);
+  else viscous_kernel<false, false><<<grid, bx, 0, st>>>(P, prim, grad, R, accumulate);
   return cudaGetLastError();
 }
 

@@ -62,9 +62,12 @@ def test_layout_alignment_and_sizes(osbli):
     p = osbli.make_params(n=(512, 512, 512), visc=osbli.VISC_CONST)
     lay = osbli.osbli_get_layout(p)
     assert 5.3e9 < lay.total_doubles * 8 < 6.2e9                          # "about 5.4 GB per state" + halos
-    assert osbli.osbli_workspace_bytes(p) == 19 * lay.stride_var * 8      # R + Q2 + Q3 + u, v, w, T
+    assert osbli.osbli_workspace_bytes(p) == 15 * lay.stride_var * 8      # R + Q2 + Q3 (the fast viscous path stages nothing)
+    ex = ((osbli.BC_EXTRAP0,) * 2,) * 3
+    assert osbli.osbli_workspace_bytes(osbli.make_params(n=(512, 512, 512), visc=osbli.VISC_CONST, bc=ex)) == 31 * lay.stride_var * 8
+    assert osbli.osbli_workspace_bytes(osbli.make_params(n=(512, 512, 512), visc=osbli.VISC_SUTHERLAND, bc=ex)) == 35 * lay.stride_var * 8
     p = osbli.make_params(n=(64, 64, 64), visc=osbli.VISC_SUTHERLAND)
-    assert osbli.osbli_workspace_bytes(p) == 20 * osbli.osbli_get_layout(p).stride_var * 8
+    assert osbli.osbli_workspace_bytes(p) == 35 * osbli.osbli_get_layout(p).stride_var * 8   # + u, v, w, T, mu and their 15 first differences
     p = osbli.make_params(n=(64, 1, 1))
     assert osbli.osbli_workspace_bytes(p) == 15 * osbli.osbli_get_layout(p).stride_var * 8
 
