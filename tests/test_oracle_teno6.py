@@ -119,3 +119,45 @@ def test_residual_conservation_and_reflection():
     R5 = O.Oracle(**{**case.physics(), "scheme": W.TENO5})
     R5 = R5.interior(R5.rhs(R5.bc(case.Q0.copy())))
     assert 1e-9 < np.abs(R5 - R).max() < 1e-2
+
+
+def test_beta3_evaluation_form_decides_cutoffs_on_flat_data():
+    """DESIGN.md Q32 / Q14: TENO6's cut-off is evaluation-form sensitive.  The oracle evaluates beta_3 from the Taylor
+    coefficients of the cubic (sum of squares of difference combinations, like the printed eq. (17)-(19)); the
+    expanded literature polynomial (2107 c^2 - 9402 cd + ... + 547 f^2)/240 is the same quadratic form but cancels to
+    ~1e-14 on O(1) data -- above eps = 1e-16 -- so in the constant states of the developed Sod problem it fabricates a
+    tau_6 that cuts stencils.  Component-wise proxy on rho, rho u, rho E of the oracle's state at t = 0.03 (both
+    orientations): a large share of the six-point windows changes a cut-off decision between the two forms, nearly
+    all of them where the data is flat to 1e-10."""
+    import numpy as np
+    case = W.sod(scheme=W.TENO6)
+    orc = O.Oracle(**case.physics())
+    Q = orc.run(case.Q0.copy(), case.dt, 150)
+
+    def cut(a, b, c, d, e, f, taylor):
+        s0, t0, s1, t1, s2, t2 = c - 2 * d + e, 3 * c - 4 * d + e, b - 2 * c + d, b - d, a - 2 * b + c, a - 4 * b + 3 * c
+        b0, b1, b2 = 13 / 12 * s0 * s0 + 0.25 * t0 * t0, 13 / 12 * s1 * s1 + 0.25 * t1 * t1, 13 / 12 * s2 * s2 + 0.25 * t2 * t2
+        if taylor:
+            a1, a2, a3 = (-43 * c + 69 * d - 33 * e + 7 * f) / 24, (2 * c - 5 * d + 4 * e - f) / 2, (-c + 3 * d - 3 * e + f) / 6
+            b3 = a1 * a1 + 13 / 3 * a2 * a2 + 3129 / 80 * a3 * a3 + 0.5 * a1 * a3
+        else:
+            b3 = (c * (2107 * c - 9402 * d + 7042 * e - 1854 * f) + d * (11003 * d - 17246 * e + 4642 * f)
+                  + e * (7043 * e - 3882 * f) + 547 * f * f) / 240
+        tau = np.abs(b3 - (b0 + b2 + 4 * b1) / 6)
+        g = [(1 + tau / (x + 1e-16)) ** 6 for x in (b0, b1, b2, b3)]
+        return np.array([x / sum(g) < 1e-6 for x in g])
+
+    windows = flips = flat = 0
+    for comp in (0, 1, 4):
+        for orient in (1, -1):
+            v = Q[comp, 0, 0, ::orient]
+            w = [v[m:len(v) - 5 + m] for m in range(6)]
+            differ = (cut(*w, True) != cut(*w, False)).any(axis=0)
+            spread = np.max(w, axis=0) - np.min(w, axis=0)
+            flat += int((spread[differ] < 1e-10).sum())
+            windows += differ.size
+            flips += int(differ.sum())
+    print(windows, flips, flat)
+    assert windows == 2406 and flips > 100 and flat > 0.8 * flips, (windows, flips, flat)   # 411 flips on the reference build
+    # the oracle's own indicator is exactly zero on constant data (no fabricated tau)
+    assert np.all(O.teno6_indicators(1.0, 1.0, 1.0, 1.0, 1.0, 1.0) == 0.0)
