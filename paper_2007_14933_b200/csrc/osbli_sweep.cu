@@ -37,7 +37,9 @@ __global__ void __launch_bounds__(128, CURV ? 1 : OSBLI_YZ_MINB)
 sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
                 int chunk, const RkArgs rk) {
   static_assert(DIR == 1 || DIR == 2, "x has its own kernel");
-  __shared__ double stg[8][5][128];     // per-thread slots: R (0-2) and dU (3-5) of nodes n % 3, raw state (6-7) of nodes n & 1
+  __shared__ double stg[CURV ? 6 : 8][5][128];   // per-thread slots: R (0-2) and dU (3-5) of nodes n % 3, raw state (6-7) of nodes n & 1
+  __shared__ double kring[CURV ? 18 : 1][128];    // curvilinear: K_m of the six window points (KRing)
+  KRing<128> KR{&kring[0][threadIdx.x], 0};
   const Layout &Ly = P.L;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= Ly.n[0]) return;
@@ -86,6 +88,7 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
     load(s0 - 4 + m, q, K);
     double rs;
     make_point<DIR, CURV>(P, q[0], q[1], q[2], q[3], q[4], K[0], K[1], K[2], w[m], rs);
+    if constexpr (CURV) KR.put(m, K[0], K[1], K[2]);
     if (m >= 3) rsq[m - 3] = rs;
     if (m == 3) rl = roe_side<CURV>(P, w[3], rs);   // node s0-1 = left node of the first interface
   }
@@ -135,6 +138,7 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
       for (int c = 0; c < 5; ++c) qn[c] = stg[6 + ((q + 3) & 1)][c][threadIdx.x];
     }
     make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], w[5], rsq[2]);
+    if constexpr (CURV) { KR.advance(); KR.put(5, Kn[0], Kn[1], Kn[2]); }
     if constexpr (!kAsyncQ) {
       if (q + 1 < s1) load(q + 4, qn, Kn);       // node (q+1)+3, used by the next interface
     }
@@ -143,7 +147,7 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
     double rold[5] = {0, 0, 0, 0, 0};
     const RoeSide rr = roe_side<CURV>(P, w[3], rsq[0]);
     double f[5];
-    if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, rl, rr, rp, f);
+    if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, KR, rl, rr, rp, f);
     else interface_flux<DIR, SCHEME>(P, w, rl, rr, rp, f);
     rl = rr;
     if (q >= s0) {
@@ -215,6 +219,7 @@ constexpr int kXWarps = 4;             // warps per block
 template <bool CURV> struct XSmem {
   double in[CURV ? 9 : 5][32][kXP];    // staged rows: 5 conservative variables (+ detJ, K_x, K_y, K_z)
   double out[5][32][kXP];              // staged flux differences
+  double K[CURV ? 18 : 1][32];         // curvilinear: K_m of the six window points of every lane (KRing)
 };
 
 template <int SCHEME, bool CURV>
@@ -273,6 +278,11 @@ sweep_x_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q
   };
 
   Pt<CURV> w[6];
+  KRing<32> KR{&S.K[0][lane], 0};
+  if constexpr (CURV) {
+#pragma unroll
+    for (int m = 0; m < 6; ++m) KR.put(m, 1.0, 0.0, 0.0);        // placeholders until six real points have entered
+  }
   double rsq[3] = {1.0, 1.0, 1.0};
   double Jw[4] = {1.0, 1.0, 1.0, 1.0};           // detJ of window slots 2..5 (curvilinear divisor)
   RoeSide rl = {0, 0, 0, 0, 0};
@@ -306,13 +316,14 @@ sweep_x_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q
         Jw[3] = J;
       }
       make_point<0, CURV>(P, r, mx, my, mz, E, kx, ky, kz, w[5], rsq[2]);
+      if constexpr (CURV) { KR.advance(); KR.put(5, kx, ky, kz); }
     }
     const int q = node - 3;                                      // interface q+1/2 is now computable
     if (q == s0 - 2) rl = roe_side<CURV>(P, w[3], rsq[0]);         // slot 3 holds node s0-1
     if (q < s0 - 1) continue;
     const RoeSide rr = roe_side<CURV>(P, w[3], rsq[0]);
     double f[5];
-    if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, rl, rr, rp, f);
+    if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, KR, rl, rr, rp, f);
     else interface_flux<0, SCHEME>(P, w, rl, rr, rp, f);
     rl = rr;
     if (q >= s0) {
