@@ -91,15 +91,32 @@ gradients_kernel(const __grid_constant__ DevParams P, const double *__restrict__
     for (int f = 0; f < NF; ++f) {
       double acc = 0.0;
 #pragma unroll
-      for (int m = 0; m < 5; ++m)
-        if (a[m] != 0.0) acc = fma(a[m] * sc, __ldg(prim + f * sv + at + (long long)(o + m) * st[l]), acc);
+      for (int m = 0; m < 5; ++m) acc = fma(a[m] * sc, __ldg(prim + f * sv + at + (long long)(o + m) * st[l]), acc);
       grad[(f * 3 + l) * sv + at] = acc;
     }
   }
 }
 
+// Stencil tables (times 12 Delta resp. 12 Delta^2) by node class: 0 interior eq. (28)/(29), 1..4 the one-sided
+// closures eq. (30)-(35) at nodes 0, 1, n-2, n-1; c_off = offset of the first stencil node.  Kept in constant memory
+// and indexed by the class of the node so that no coefficient array waits in registers.
+static __constant__ double c_d1[5][5] = {{1.0, -8.0, 0.0, 8.0, -1.0}, {-25.0, 48.0, -36.0, 16.0, -3.0}, {-3.0, -10.0, 18.0, -6.0, 1.0},
+                                         {-1.0, 6.0, -18.0, 10.0, 3.0}, {3.0, -16.0, 36.0, -48.0, 25.0}};
+static __constant__ double c_d2[5][5] = {{-1.0, 16.0, -30.0, 16.0, -1.0}, {35.0, -104.0, 114.0, -56.0, 11.0}, {11.0, -20.0, 6.0, 4.0, -1.0},
+                                         {-1.0, 4.0, 6.0, -20.0, 11.0}, {11.0, -56.0, 114.0, -104.0, 35.0}};
+static __constant__ int c_off[5] = {-2, 0, -1, -3, -4};
+__device__ __forceinline__ int node_class(int n, int i, int per) {
+  if (per) return 0;
+  return i == 0 ? 1 : (i == 1 ? 2 : (i == n - 2 ? 3 : (i == n - 1 ? 4 : 0)));
+}
+
+// One thread per node.  Written so that little waits in registers (the first version held the coefficient
+// arrays, all first and all second differences of all fields at once: 206 registers, 8 warps per SM, every load a
+// full-latency stall): the physical first derivatives of u, v, w, T (, mu) are formed from the stored first
+// differences; then ONE field at a time its second / mixed differences are formed and folded straight into the
+// Laplacians and into d_i(div u).
 template <bool CURV, bool SUTH>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 3)
 viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ prim, const double *__restrict__ grad,
                double *__restrict__ R, int accumulate) {
   const Layout &L = P.L;
@@ -110,30 +127,52 @@ viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ p
   const long long sv = L.sv;
   const long long st[3] = {1, L.sy, L.sz};
   bool act[3];
-  double a1[3][5], a2[3][5];
-  int o1[3], o2[3];
+  int cls[3];
+  double s1[3], s2[3];
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
     act[k] = L.n[k] > 1;
-    o1[k] = d1_stencil(L.n[k], nd[k], P.periodic[k], a1[k]);
-    o2[k] = d2_stencil(L.n[k], nd[k], P.periodic[k], a2[k]);
-    const double s1 = CURV ? (1.0 / 12.0) : P.inv12d[k];
-    const double s2 = CURV ? (1.0 / 12.0) : P.inv12d2[k];
-#pragma unroll
-    for (int m = 0; m < 5; ++m) { a1[k][m] *= s1; a2[k][m] *= s2; }
+    cls[k] = node_class(L.n[k], nd[k], P.periodic[k]);
+    s1[k] = CURV ? (1.0 / 12.0) : P.inv12d[k];
+    s2[k] = CURV ? (1.0 / 12.0) : P.inv12d2[k];
   }
   auto F = [&](int f, long long off) { return __ldg(prim + f * sv + at + off); };
-
-  // computational differences: c1[f][k] = delta_k f (stored by gradients_kernel), c2[f][k][l] = delta_kl f
-  constexpr int NF1 = SUTH ? 5 : 4;
   auto Gd = [&](int f, int l, long long off) { return __ldg(grad + (f * 3 + l) * sv + at + off); };
-  double c1[5][3], c2[4][3][3];
+  constexpr int NF1 = SUTH ? 5 : 4;
+  constexpr int IJ[3][3] = {{0, 1, 2}, {1, 3, 4}, {2, 4, 5}};
+  // the residual this kernel adds to: requested first, consumed last
+  double rold[4] = {0.0, 0.0, 0.0, 0.0};
+  if (accumulate) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c) rold[c] = R[(c + 1) * sv + at];
+  }
+
+  double D[3][3];
+  if constexpr (CURV) {
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+#pragma unroll
+      for (int j = 0; j < 3; ++j) D[k][j] = __ldg(P.D[k][j] + at);
+  }
+  // computational first differences c1[f][k] = delta_k f (stored by gradients_kernel) and physical first derivatives
+  double c1[5][3], g1[5][3];
 #pragma unroll
   for (int f = 0; f < 5; ++f)
 #pragma unroll
     for (int k = 0; k < 3; ++k) c1[f][k] = (f < NF1 && act[k]) ? Gd(f, k, 0) : 0.0;
 #pragma unroll
-  for (int f = 0; f < 4; ++f)
+  for (int f = 0; f < 5; ++f)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      if constexpr (CURV) g1[f][j] = fma(D[0][j], c1[f][0], fma(D[1][j], c1[f][1], D[2][j] * c1[f][2]));
+      else g1[f][j] = c1[f][j];
+    }
+
+  // second derivatives, one field at a time: lap[f] = sum_j d_jj f;  gdiv[a] = d_a(d_k u_k) = sum_f d_a d_f u_f
+  double lap[4], gdiv[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+  for (int f = 0; f < 4; ++f) {
+    double c2[3][3];
 #pragma unroll
     for (int k = 0; k < 3; ++k)
 #pragma unroll
@@ -142,64 +181,42 @@ viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ p
         // uniform grids only need d_i d_k u_k: mixed terms of velocity component f along (f, other)
         const bool needed = CURV || k == l || (f < 3 && (k == f || l == f));
         if (needed && act[k] && act[l]) {
+          const int o = c_off[cls[k]];
           if (k == l) {
 #pragma unroll
-            for (int m = 0; m < 5; ++m) acc = fma(a2[k][m], F(f, (long long)(o2[k] + m) * st[k]), acc);
+            for (int m = 0; m < 5; ++m) acc = fma(c_d2[cls[k]][m] * s2[k], F(f, (long long)(o + m) * st[k]), acc);
           } else {
             // delta_k (delta_l f), k < l: the first-difference stencil along k over the stored delta_l f
 #pragma unroll
-            for (int a = 0; a < 5; ++a)
-              if (a1[k][a] != 0.0) acc = fma(a1[k][a], Gd(f, l, (long long)(o1[k] + a) * st[k]), acc);
+            for (int m = 0; m < 5; ++m)     // no test for the zero centre coefficient: a predicate in front of the load keeps it from being hoisted
+              acc = fma(c_d1[cls[k]][m] * s1[k], Gd(f, l, (long long)(o + m) * st[k]), acc);
           }
         }
-        c2[f][k][l] = acc;
-        c2[f][l][k] = acc;
+        c2[k][l] = acc;
+        c2[l][k] = acc;
       }
-
-  // physical derivatives g1[f][j] = d_j f, g2[f][i][j] = d_i d_j f
-  double g1[5][3], g2[4][3][3];
-  if constexpr (!CURV) {
+    // physical d_a d_b f for the (a, b) that are used: the diagonal, and (a, f) for the velocity components
+    auto g2 = [&](int a_, int b_) {
+      if constexpr (!CURV) return c2[a_][b_];
+      else {
+        double acc = 0.0;
 #pragma unroll
-    for (int f = 0; f < 5; ++f)
+        for (int k = 0; k < 3; ++k)
 #pragma unroll
-      for (int j = 0; j < 3; ++j) g1[f][j] = c1[f][j];
+          for (int l = 0; l < 3; ++l) acc = fma(D[k][a_] * D[l][b_], c2[k][l], acc);
 #pragma unroll
-    for (int f = 0; f < 4; ++f)
+        for (int l = 0; l < 3; ++l) acc = fma(__ldg(P.E[l][IJ[a_][b_]] + at), c1[f][l], acc);
+        return acc;
+      }
+    };
+    double dg[3];
 #pragma unroll
-      for (int a = 0; a < 3; ++a)
+    for (int a_ = 0; a_ < 3; ++a_) dg[a_] = g2(a_, a_);
+    lap[f] = dg[0] + dg[1] + dg[2];
+    if (f < 3) {
 #pragma unroll
-        for (int b = 0; b < 3; ++b) g2[f][a][b] = c2[f][a][b];
-  } else {
-    constexpr int IJ[3][3] = {{0, 1, 2}, {1, 3, 4}, {2, 4, 5}};
-    double D[3][3], E[3][6];
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-#pragma unroll
-      for (int j = 0; j < 3; ++j) D[k][j] = __ldg(P.D[k][j] + at);
-#pragma unroll
-      for (int m = 0; m < 6; ++m) E[k][m] = __ldg(P.E[k][m] + at);
+      for (int a_ = 0; a_ < 3; ++a_) gdiv[a_] += (a_ == f) ? dg[f] : g2(a_, f);
     }
-#pragma unroll
-    for (int f = 0; f < 5; ++f)
-#pragma unroll
-      for (int j = 0; j < 3; ++j)
-        g1[f][j] = fma(D[0][j], c1[f][0], fma(D[1][j], c1[f][1], D[2][j] * c1[f][2]));
-#pragma unroll
-    for (int f = 0; f < 4; ++f)
-#pragma unroll
-      for (int a = 0; a < 3; ++a)
-#pragma unroll
-        for (int b = a; b < 3; ++b) {
-          double acc = 0.0;
-#pragma unroll
-          for (int k = 0; k < 3; ++k)
-#pragma unroll
-            for (int l = 0; l < 3; ++l) acc = fma(D[k][a] * D[l][b], c2[f][k][l], acc);
-#pragma unroll
-          for (int l = 0; l < 3; ++l) acc = fma(E[l][IJ[a][b]], c1[f][l], acc);
-          g2[f][a][b] = acc;
-          g2[f][b][a] = acc;
-        }
   }
 
   const double vel[3] = {F(0, 0), F(1, 0), F(2, 0)};
@@ -209,9 +226,7 @@ viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ p
   double M[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
-    const double lap = g2[a][0][0] + g2[a][1][1] + g2[a][2][2];
-    const double gdiv = g2[0][a][0] + g2[1][a][1] + g2[2][a][2];
-    double m = mu * fma(gdiv, 1.0 / 3.0, lap);
+    double m = mu * fma(gdiv[a], 1.0 / 3.0, lap[a]);
     if constexpr (SUTH) {
       double cross = 0.0;
 #pragma unroll
@@ -230,19 +245,15 @@ viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ p
       phi = fma(s, g1[a][b], phi);
     }
   phi *= mu * P.inv_Re;
-  const double lapT = g2[3][0][0] + g2[3][1][1] + g2[3][2][2];
-  double heat = mu * lapT;
+  double heat = mu * lap[3];
   if constexpr (SUTH) heat += g1[4][0] * g1[3][0] + g1[4][1] * g1[3][1] + g1[4][2] * g1[3][2];
   heat *= P.cq;
 
   const double r1 = M[0] * P.inv_Re, r2 = M[1] * P.inv_Re, r3 = M[2] * P.inv_Re;
   const double r4 = fma(vel[0], r1, fma(vel[1], r2, vel[2] * r3)) + phi + heat;
   double *dst = R + sv + at;
-  if (accumulate) {
-    dst[0] += r1; dst[sv] += r2; dst[2 * sv] += r3; dst[3 * sv] += r4;
-  } else {
-    R[at] = 0.0; dst[0] = r1; dst[sv] = r2; dst[2 * sv] = r3; dst[3 * sv] = r4;
-  }
+  if (!accumulate) R[at] = 0.0;
+  dst[0] = rold[0] + r1; dst[sv] = rold[1] + r2; dst[2 * sv] = rold[2] + r3; dst[3 * sv] = rold[3] + r4;
 }
 
 // ---------------------------------------------------------------------------------------------
