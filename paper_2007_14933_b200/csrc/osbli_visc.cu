@@ -115,24 +115,23 @@ __device__ __forceinline__ int node_class(int n, int i, int per) {
 // full-latency stall): the physical first derivatives of u, v, w, T (, mu) are formed from the stored first
 // differences; then ONE field at a time its second / mixed differences are formed and folded straight into the
 // Laplacians and into d_i(div u).
-template <bool CURV, bool SUTH>
-__global__ void __launch_bounds__(128, 3)
-viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ prim, const double *__restrict__ grad,
-               double *__restrict__ R, int accumulate) {
+// INTERIOR: the node uses the interior stencils eq. (28)-(29) in every direction (all but the two nodes next to each
+// non-periodic boundary): coefficients and offsets are compile-time constants, nothing is fetched from the tables.
+template <bool CURV, bool SUTH, bool INTERIOR>
+__device__ __forceinline__ void viscous_node(const DevParams &P, const double *__restrict__ prim, const double *__restrict__ grad,
+                                             double *__restrict__ R, int accumulate, const int (&nd)[3], const int (&cls_in)[3]) {
   const Layout &L = P.L;
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= L.n[0]) return;
-  const int nd[3] = {i, (int)blockIdx.y, (int)blockIdx.z};
   const long long at = L.at(nd[0], nd[1], nd[2]);
   const long long sv = L.sv;
   const long long st[3] = {1, L.sy, L.sz};
+  constexpr double kD1[5] = {1.0, -8.0, 0.0, 8.0, -1.0}, kD2[5] = {-1.0, 16.0, -30.0, 16.0, -1.0};
   bool act[3];
   int cls[3];
   double s1[3], s2[3];
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
     act[k] = L.n[k] > 1;
-    cls[k] = node_class(L.n[k], nd[k], P.periodic[k]);
+    cls[k] = INTERIOR ? 0 : cls_in[k];
     s1[k] = CURV ? (1.0 / 12.0) : P.inv12d[k];
     s2[k] = CURV ? (1.0 / 12.0) : P.inv12d2[k];
   }
@@ -181,15 +180,19 @@ viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ p
         // uniform grids only need d_i d_k u_k: mixed terms of velocity component f along (f, other)
         const bool needed = CURV || k == l || (f < 3 && (k == f || l == f));
         if (needed && act[k] && act[l]) {
-          const int o = c_off[cls[k]];
+          const int o = INTERIOR ? -2 : c_off[cls[k]];
           if (k == l) {
 #pragma unroll
-            for (int m = 0; m < 5; ++m) acc = fma(c_d2[cls[k]][m] * s2[k], F(f, (long long)(o + m) * st[k]), acc);
+            for (int m = 0; m < 5; ++m)
+              acc = fma((INTERIOR ? kD2[m] : c_d2[cls[k]][m]) * s2[k], F(f, (long long)(o + m) * st[k]), acc);
           } else {
-            // delta_k (delta_l f), k < l: the first-difference stencil along k over the stored delta_l f
+            // delta_k (delta_l f), k < l: the first-difference stencil along k over the stored delta_l f.  Closures: no
+            // run-time test for a zero coefficient (a predicate in front of a load keeps it from being hoisted)
 #pragma unroll
-            for (int m = 0; m < 5; ++m)     // no test for the zero centre coefficient: a predicate in front of the load keeps it from being hoisted
-              acc = fma(c_d1[cls[k]][m] * s1[k], Gd(f, l, (long long)(o + m) * st[k]), acc);
+            for (int m = 0; m < 5; ++m) {
+              if (INTERIOR && m == 2) continue;
+              acc = fma((INTERIOR ? kD1[m] : c_d1[cls[k]][m]) * s1[k], Gd(f, l, (long long)(o + m) * st[k]), acc);
+            }
           }
         }
         c2[k][l] = acc;
@@ -254,6 +257,21 @@ viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ p
   double *dst = R + sv + at;
   if (!accumulate) R[at] = 0.0;
   dst[0] = rold[0] + r1; dst[sv] = rold[1] + r2; dst[2 * sv] = rold[2] + r3; dst[3 * sv] = rold[3] + r4;
+}
+
+template <bool CURV, bool SUTH>
+__global__ void __launch_bounds__(128, 3)
+viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ prim, const double *__restrict__ grad,
+               double *__restrict__ R, int accumulate) {
+  const Layout &L = P.L;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= L.n[0]) return;
+  const int nd[3] = {i, (int)blockIdx.y, (int)blockIdx.z};
+  int cls[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) cls[k] = node_class(L.n[k], nd[k], P.periodic[k]);
+  if ((cls[0] | cls[1] | cls[2]) == 0) viscous_node<CURV, SUTH, true>(P, prim, grad, R, accumulate, nd, cls);
+  else viscous_node<CURV, SUTH, false>(P, prim, grad, R, accumulate, nd, cls);
 }
 
 // ---------------------------------------------------------------------------------------------

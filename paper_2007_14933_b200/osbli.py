@@ -276,31 +276,41 @@ class Solver:
     def _stream(self):
         return self.torch.cuda.current_stream(self.device).cuda_stream
 
+    def _on_device(self):
+        """The handle's device made current for the duration of a call (launches go to the current device)."""
+        return self.torch.cuda.device(self.device)
+
     def bc(self, Q):
-        osbli_bc(self.handle, Q.data_ptr(), self._stream())
+        with self._on_device():
+            osbli_bc(self.handle, Q.data_ptr(), self._stream())
         return Q
 
     def rhs(self, Q, R=None):
         if R is None:
             R = self.empty_state(0.0)
-        osbli_rhs(self.handle, Q.data_ptr(), R.data_ptr(), self._stream())
+        with self._on_device():
+            osbli_rhs(self.handle, Q.data_ptr(), R.data_ptr(), self._stream())
         return R
 
     def rk3_step(self, Q, Qtmp, dt):
-        osbli_rk3_step(self.handle, Q.data_ptr(), Qtmp.data_ptr(), dt, self._stream())
+        with self._on_device():
+            osbli_rk3_step(self.handle, Q.data_ptr(), Qtmp.data_ptr(), dt, self._stream())
         return Q
 
     def rk4_step(self, Q, Qtmp, dt):
-        osbli_rk4_step(self.handle, Q.data_ptr(), Qtmp.data_ptr(), dt, self._stream())
+        with self._on_device():
+            osbli_rk4_step(self.handle, Q.data_ptr(), Qtmp.data_ptr(), dt, self._stream())
         return Q
 
     def advance_host(self, hQ, Q, Qtmp, dt, nsteps):
-        osbli_advance_host(self.handle, hQ.data_ptr(), Q.data_ptr(), Qtmp.data_ptr(), dt, nsteps, self._stream())
+        with self._on_device():
+            osbli_advance_host(self.handle, hQ.data_ptr(), Q.data_ptr(), Qtmp.data_ptr(), dt, nsteps, self._stream())
         return hQ
 
     def advance_host_batch(self, hQs, Qs, Qtmp, dt, nsteps):
-        osbli_advance_host_batch(self.handle, [t.data_ptr() for t in hQs], [t.data_ptr() for t in Qs], Qtmp.data_ptr(),
-                                 dt, nsteps, self._stream())
+        with self._on_device():
+            osbli_advance_host_batch(self.handle, [t.data_ptr() for t in hQs], [t.data_ptr() for t in Qs], Qtmp.data_ptr(),
+                                     dt, nsteps, self._stream())
         return hQs
 
     def profile_begin(self):
