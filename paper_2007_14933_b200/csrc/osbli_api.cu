@@ -136,7 +136,10 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
     if (rk) return OSBLI_EINVAL;
     OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X, st, launch_central(P, Q, R, st));
     if (fast_visc) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous_fast(P, Q, R, &h->tmaps, st));
-    else if (P.visc != OSBLI_VISC_NONE) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, 1, st));
+    else if (P.visc != OSBLI_VISC_NONE) {
+      OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, 1, st));
+      ++h->launches;                                                // launch_viscous = gradients_kernel + viscous_kernel
+    }
     if (P.has_force) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_force(P, Q, R, st));
     return OSBLI_OK;
   }
@@ -148,14 +151,20 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
     if (P.L.n[d] <= 1) continue;
     if (d == last && last > 0) {                                    // viscous terms go in front of the last sweep
       if (fast_visc) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous_fast(P, Q, R, &h->tmaps, st));
-      else if (P.visc != OSBLI_VISC_NONE) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, accumulate, st));
+      else if (P.visc != OSBLI_VISC_NONE) {
+        OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, accumulate, st));
+        ++h->launches;                                              // launch_viscous = gradients_kernel + viscous_kernel
+      }
       if (P.has_force) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_force(P, Q, R, st));
     }
     OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep(P, d, Q, R, accumulate, d == last ? rk : nullptr, st));
     accumulate = 1;
   }
   if (last == 0 && P.visc != OSBLI_VISC_NONE)                       // 1-D: the x sweep, then the viscous terms
+  {
     OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, accumulate, st));
+    ++h->launches;                                                  // launch_viscous = gradients_kernel + viscous_kernel
+  }
   if (last == 0 && P.has_force) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_force(P, Q, R, st));
   return OSBLI_OK;
 }
