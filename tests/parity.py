@@ -157,4 +157,5 @@ def check_residual(name, case, Qi, Rg_i, Ro_i, metrics=None, margin_i=None, marg
         assert err[c] <= tol[c], (f"{name}: variable {c}: |dR| = {err[c]:.3e} > tol {tol[c]:.3e} "
                                   f"(1e-11 rel = {tol_rel[c]:.3e}, rounding floor x{K_ULP:g} = {tol_floor[c]:.3e}; "
                                   f"q28 = {rel[c]:.3e})")
+    check_residual.last = {"q28": rel, "floor_units": (err / (tol_floor / K_ULP)).tolist(), "excluded_nodes": nflip}
     return err, tol
