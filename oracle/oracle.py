@@ -3,7 +3,7 @@
 TEST INFRASTRUCTURE, NOT PRODUCT CODE.  Only tests/, __graft_entry__.smoke() and bench.py's
 cpu_baseline / --impl reference legs may import this module.  It imports nothing from the CUDA
 package; it takes plain numpy arrays in the oracle's own dense layout
-([5][NZ][NY][NX], halo 3 in every active direction, see osbli_oracle.h).
+([5][NZ][NY][NX], halo 3 in every active direction, 4 for the 7th-order scheme, see osbli_oracle.h).
 """
 from __future__ import annotations
 
@@ -19,7 +19,7 @@ _SRC = _HERE / "osbli_oracle.cpp"
 _HDR = _HERE / "osbli_oracle.h"
 _LIB = _HERE / "libosbli_oracle.so"
 
-WENOZ5, TENO5, TENO6, WENOJS5, CENTRAL4, WENOZ3 = 0, 1, 2, 3, 4, 5
+WENOZ5, TENO5, TENO6, WENOJS5, CENTRAL4, WENOZ3, WENOZ7 = 0, 1, 2, 3, 4, 5, 6
 VISC_NONE, VISC_CONST, VISC_SUTHERLAND = 0, 1, 2
 BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL = 0, 1, 2, 3
 PART_INVISCID, PART_VISCOUS = 1, 2
@@ -76,6 +76,8 @@ def lib():
         L.oracle_reconstruct.argtypes = [C.c_int32] + [C.c_double] * 7 + [_dp]
         L.oracle_reconstruct6.restype = C.c_double
         L.oracle_reconstruct6.argtypes = [C.c_double] * 8 + [_dp]
+        L.oracle_reconstruct7.restype = C.c_double
+        L.oracle_reconstruct7.argtypes = [_dp, C.c_double, _dp]
         L.oracle_teno6_indicators.restype = None
         L.oracle_teno6_indicators.argtypes = [C.c_double] * 6 + [_dp]
         L.oracle_eigensystem.restype = None
@@ -131,6 +133,15 @@ def reconstruct6(a, b, c, d, e, f, eps=1e-16, ct=1e-6, with_margin=False):
     return (v, m.value) if with_margin else v
 
 
+def reconstruct7(v7, eps=1e-16, with_indicators=False):
+    """WENO-7Z value at i+1/2 from the seven nodes i-3..i+3; optionally (beta_0..beta_3, tau_7)."""
+    v = np.ascontiguousarray(v7, dtype=np.float64)
+    assert v.shape == (7,)
+    out = np.zeros(5)
+    val = lib().oracle_reconstruct7(_ptr(v), eps, _ptr(out))
+    return (val, out) if with_indicators else val
+
+
 def teno6_indicators(a, b, c, d, e, f):
     out = np.zeros(5)
     lib().oracle_teno6_indicators(a, b, c, d, e, f, _ptr(out))
@@ -176,15 +187,16 @@ def rk3_update(s, dt, U, dU, R):
     lib().oracle_rk3_update(int(s), float(dt), U.size, _ptr(U), _ptr(dU), _ptr(R))
 
 
-def metrics_from_coords(coords, n, periodic, delta=(1.0, 1.0, 1.0), nthreads=None):
+def metrics_from_coords(coords, n, periodic, delta=(1.0, 1.0, 1.0), nthreads=None, scheme=WENOZ5):
     """PAPER.md:228 metric terms from node coordinates.
 
     coords: [3, NZ, NY, NX] (x, y, z on the halo-extended grid, periodic continuation in the
     halos of periodic directions).  Returns {"D": 3x3 list, "detJ": field, "E": 3x6 list} of
-    halo-filled fields in oracle layout.
+    halo-filled fields in oracle layout.  `scheme` only selects the halo depth (4 for WENO-7Z).
     """
     coords = np.ascontiguousarray(coords, dtype=np.float64)
     p = _Params()
+    p.scheme = int(scheme)
     p.n[:] = [int(v) for v in n]
     p.delta[:] = [float(v) for v in delta]
     for d in range(3):
@@ -211,7 +223,7 @@ class Oracle:
                  bc=((0, 0), (0, 0), (0, 0)), wall_T=((0, 0), (0, 0), (0, 0)), dirichlet=None,
                  nthreads=None, force=(0.0, 0.0, 0.0), averaging=AVG_ROE, rk3_form=RK3_WILLIAMSON):
         self.n = tuple(int(v) for v in n)
-        self.h = tuple(3 if v > 1 else 0 for v in self.n)
+        self.h = tuple((4 if int(scheme) == WENOZ7 else 3) if v > 1 else 0 for v in self.n)      # = oracle_halo()
         self.N = tuple(v + 2 * h for v, h in zip(self.n, self.h))
         self.shape = (5, self.N[2], self.N[1], self.N[0])
         self.fshape = self.shape[1:]

@@ -37,7 +37,8 @@ Grid make_grid(const oracle_params *p) {
   Grid g;
   for (int d = 0; d < 3; ++d) {
     g.n[d] = p->n[d];
-    g.h[d] = p->n[d] > 1 ? 3 : 0;
+    /* ghost points: 3 for the 5th/6th-order stencils, 4 for the 7th-order one (i-3..i+4) */
+    g.h[d] = p->n[d] > 1 ? (p->scheme == ORACLE_WENOZ7 ? 4 : 3) : 0;
     g.N[d] = g.n[d] + 2 * g.h[d];
   }
   g.total = (long)g.N[0] * g.N[1] * g.N[2];
@@ -285,15 +286,57 @@ void normal_at(const oracle_params *p, int dir, long at, double *K) {
   }
 }
 
+/* ------------------------------------------------------------ WENO-7Z reconstruction ---- */
+/* Seventh-order WENO-Z (k = 4 in eq. (15), (20), (22); "any arbitrary odd order", used at 7th order
+ * in PAPER.md:485-495 and 531-533).  v[0..6] = nodes i-3..i+3, value at i+1/2.  Candidate r lives on the four
+ * nodes {i-r .. i-r+3}, r = 0..3 (r = 0 the most downwind one, as beta_0 of eq. (17)), and is the cubic with those
+ * cell averages evaluated at the interface; the ideal weights d_r = (4, 18, 12, 1)/35 [18] combine them to the
+ * 7th-order value (-3, 25, -101, 319, 214, -38, 4)/420.  beta_r: eq. (16) on the cubic, written as for TENO6
+ * (a_1^2 + 13/3 a_2^2 + 3129/80 a_3^2 + a_1 a_3 / 2 with the Taylor coefficients of the cubic at the centre of
+ * cell i).  tau_7 = |beta_0 - beta_3|, "the absolute difference in the smoothness indicators over the full
+ * reconstruction stencil" (Q40).  Weights eq. (22). */
+double reconstruct7(const double *v, double eps, double *indicators = nullptr) {
+  const double m3 = v[0], m2 = v[1], m1 = v[2], c = v[3], p1 = v[4], p2 = v[5], p3 = v[6];
+  const double q[4] = {(3.0 * c + 13.0 * p1 - 5.0 * p2 + p3) / 12.0, (-m1 + 7.0 * c + 7.0 * p1 - p2) / 12.0,
+                       (m2 - 5.0 * m1 + 13.0 * c + 3.0 * p1) / 12.0, (-3.0 * m3 + 13.0 * m2 - 23.0 * m1 + 25.0 * c) / 12.0};
+  const double dw[4] = {4.0 / 35.0, 18.0 / 35.0, 12.0 / 35.0, 1.0 / 35.0};
+  /* Taylor coefficients (first, second, third) at the centre of cell i of the four cubics */
+  const double a1[4] = {(-43.0 * c + 69.0 * p1 - 33.0 * p2 + 7.0 * p3) / 24.0, (-7.0 * m1 - 15.0 * c + 27.0 * p1 - 5.0 * p2) / 24.0,
+                        (5.0 * m2 - 27.0 * m1 + 15.0 * c + 7.0 * p1) / 24.0, (-7.0 * m3 + 33.0 * m2 - 69.0 * m1 + 43.0 * c) / 24.0};
+  const double a2[4] = {(2.0 * c - 5.0 * p1 + 4.0 * p2 - p3) / 2.0, (m1 - 2.0 * c + p1) / 2.0, (m1 - 2.0 * c + p1) / 2.0,
+                        (-m3 + 4.0 * m2 - 5.0 * m1 + 2.0 * c) / 2.0};
+  const double a3[4] = {(-c + 3.0 * p1 - 3.0 * p2 + p3) / 6.0, (-m1 + 3.0 * c - 3.0 * p1 + p2) / 6.0,
+                        (-m2 + 3.0 * m1 - 3.0 * c + p1) / 6.0, (-m3 + 3.0 * m2 - 3.0 * m1 + c) / 6.0};
+  double beta[4];
+  for (int r = 0; r < 4; ++r)
+    beta[r] = a1[r] * a1[r] + 13.0 / 3.0 * (a2[r] * a2[r]) + 3129.0 / 80.0 * (a3[r] * a3[r]) + 0.5 * (a1[r] * a3[r]);
+  const double tau = std::fabs(beta[0] - beta[3]);
+  if (indicators) {
+    for (int r = 0; r < 4; ++r) indicators[r] = beta[r];
+    indicators[4] = tau;
+  }
+  double al[4], sum = 0.0;
+  for (int r = 0; r < 4; ++r) {
+    const double x = tau / (beta[r] + eps);
+    al[r] = dw[r] * (1.0 + x * x);                          /* eq. (22) */
+    sum += al[r];
+  }
+  double val = 0.0;
+  for (int r = 0; r < 4; ++r) val += al[r] / sum * q[r];    /* eq. (15), (20) */
+  return val;
+}
+
 /* f^_{i+1/2} between node `at` and `at + stride(dir)`; PAPER.md:100-111 steps 1-2. */
 void interface_flux(const oracle_params *p, const Grid &g, const double *Q, int dir, long at,
                     double *fhat, double *margin) {
   const long s = g.stride(dir);
-  double U[6][5], F[6][5], lam0[6], lamp[6], lamm[6], K[6][3];
+  /* window: nodes i-2..i+3 (six points); the 7th-order scheme: i-3..i+4 (eight); il = window index of node i */
+  const int W = p->scheme == ORACLE_WENOZ7 ? 8 : 6, il = W / 2 - 1;
+  double U[8][5], F[8][5], lam0[8], lamp[8], lamm[8], K[8][3];
 
-  /* step 1: flux f(U_m), solution vector U_m and wave speeds at the stencil points i-2..i+3 */
-  for (int m = 0; m < 6; ++m) {
-    const long pt = at + (long)(m - 2) * s;
+  /* step 1: flux f(U_m), solution vector U_m and wave speeds at the stencil points */
+  for (int m = 0; m < W; ++m) {
+    const long pt = at + (long)(m - il) * s;
     load_state(g, Q, pt, U[m]);
     const Prim w = prim_of(p, U[m]);
     normal_at(p, dir, pt, K[m]);
@@ -313,22 +356,22 @@ void interface_flux(const oracle_params *p, const Grid &g, const double *Q, int 
    * the averaged K (uniform: e_d). */
   double nhat[3];
   {
-    const double kx = 0.5 * (K[2][0] + K[3][0]);
-    const double ky = 0.5 * (K[2][1] + K[3][1]);
-    const double kz = 0.5 * (K[2][2] + K[3][2]);
+    const double kx = 0.5 * (K[il][0] + K[il + 1][0]);
+    const double ky = 0.5 * (K[il][1] + K[il + 1][1]);
+    const double kz = 0.5 * (K[il][2] + K[il + 1][2]);
     const double kn = std::sqrt(kx * kx + ky * ky + kz * kz);
     nhat[0] = kx / kn; nhat[1] = ky / kn; nhat[2] = kz / kn;
   }
   double L[25], R[25];
-  eigensystem(p->gamma, p->averaging, U[2], U[3], nhat, L, R, nullptr);
+  eigensystem(p->gamma, p->averaging, U[il], U[il + 1], nhat, L, R, nullptr);
 
   for (int c = 0; c < 5; ++c) fhat[c] = 0.0;
   double mmin = std::numeric_limits<double>::infinity();
 
   for (int k = 0; k < 5; ++k) {
     /* step 2(c): V_k,m = l_k . U_m, G_k,m = l_k . f_m */
-    double V[6], G[6];
-    for (int m = 0; m < 6; ++m) {
+    double V[8], G[8];
+    for (int m = 0; m < W; ++m) {
       double sv = 0.0, sg = 0.0;
       for (int c = 0; c < 5; ++c) {
         sv += L[k * 5 + c] * U[m][c];
@@ -337,19 +380,25 @@ void interface_flux(const oracle_params *p, const Grid &g, const double *Q, int 
       V[m] = sv;
       G[m] = sg;
     }
-    /* step 2(d): alpha_k = max over the 6 stencil points of |lambda_k| (Q10) */
+    /* step 2(d): alpha_k = max over the stencil points of |lambda_k| (Q10) */
     const double *lam = (k < 3) ? lam0 : (k == 3 ? lamp : lamm);
     double alpha = 0.0;
-    for (int m = 0; m < 6; ++m) alpha = std::fmax(alpha, std::fabs(lam[m]));
-    double gp[6], gm[6];
-    for (int m = 0; m < 6; ++m) {
+    for (int m = 0; m < W; ++m) alpha = std::fmax(alpha, std::fabs(lam[m]));
+    double gp[8], gm[8];
+    for (int m = 0; m < W; ++m) {
       gp[m] = 0.5 * (G[m] + alpha * V[m]);          /* eq. (13) */
       gm[m] = 0.5 * (G[m] - alpha * V[m]);
     }
     /* step 2(e): g+ from the left-biased stencil, g- from its mirror image (Q4) */
     double m1, m2;
     double hp, hm;
-    if (p->scheme == ORACLE_TENO6) {
+    if (p->scheme == ORACLE_WENOZ7) {
+      double mir[7];
+      for (int m = 0; m < 7; ++m) mir[m] = gm[7 - m];
+      hp = reconstruct7(gp, p->eps);
+      hm = reconstruct7(mir, p->eps);
+      m1 = m2 = std::numeric_limits<double>::infinity();
+    } else if (p->scheme == ORACLE_TENO6) {
       hp = reconstruct6(gp[0], gp[1], gp[2], gp[3], gp[4], gp[5], p->eps, p->teno_ct, &m1);
       hm = reconstruct6(gm[5], gm[4], gm[3], gm[2], gm[1], gm[0], p->eps, p->teno_ct, &m2);
     } else {
@@ -582,7 +631,7 @@ void fill_field_halo(const oracle_params *p, const Grid &g, double *f) {
         int ijk[3];
         ijk[d] = 0; ijk[e1] = b; ijk[e2] = a;
         const long base = g.idx(ijk[0], ijk[1], ijk[2]);
-        for (int m = 1; m <= 3; ++m) {
+        for (int m = 1; m <= g.h[d]; ++m) {
           if (periodic(p, d)) {
             f[base - (long)m * s] = f[base + (long)(n - m) * s];
             f[base + (long)(n - 1 + m) * s] = f[base + (long)(m - 1) * s];
@@ -693,17 +742,17 @@ void bc_direction(const oracle_params *p, const Grid &g, double *Q, int d) {
         const long wall = base + (side == 0 ? 0 : (long)(n - 1) * s);
         const long inw = side == 0 ? s : -s;
         if (type == ORACLE_BC_PERIODIC) {
-          for (int m = 1; m <= 3; ++m)
+          for (int m = 1; m <= g.h[d]; ++m)
             for (int c = 0; c < 5; ++c) {
               double *q = Q + c * g.total;
               if (side == 0) q[base - (long)m * s] = q[base + (long)(n - m) * s];
               else           q[base + (long)(n - 1 + m) * s] = q[base + (long)(m - 1) * s];
             }
         } else if (type == ORACLE_BC_EXTRAP0) {
-          for (int m = 1; m <= 3; ++m)
+          for (int m = 1; m <= g.h[d]; ++m)
             for (int c = 0; c < 5; ++c) Q[c * g.total + wall - (long)m * inw] = Q[c * g.total + wall];
         } else if (type == ORACLE_BC_DIRICHLET) {
-          for (int m = 0; m <= 3; ++m)
+          for (int m = 0; m <= g.h[d]; ++m)
             for (int c = 0; c < 5; ++c)
               Q[c * g.total + wall - (long)m * inw] = p->dirichlet[c * g.total + wall - (long)m * inw];
         } else if (type == ORACLE_BC_WALL_ISOTHERMAL || type == ORACLE_BC_WALL_ADIABATIC) {
@@ -732,7 +781,7 @@ void bc_direction(const oracle_params *p, const Grid &g, double *Q, int d) {
           double q1[5];
           load_state(g, Q, wall + inw, q1);
           const double T1 = prim_of(p, q1).T;
-          for (int m = 1; m <= 3; ++m) {
+          for (int m = 1; m <= g.h[d]; ++m) {
             const double Tm = (m + 1) * Tw - m * T1;                       /* eq. (42) */
             const double rm = M2 * gam * pw / Tm;                          /* eq. (43) */
             double qi[5];
@@ -865,6 +914,7 @@ double oracle_reconstruct6(double a, double b, double c, double d, double e, dou
   return reconstruct6(a, b, c, d, e, f, eps, teno_ct, margin);
 }
 
+double oracle_reconstruct7(const double *v7, double eps, double *out5) { return reconstruct7(v7, eps, out5); }
 void oracle_teno6_indicators(double a, double b, double c, double d, double e, double f, double *out5) {
   reconstruct6(a, b, c, d, e, f, 1e-16, 1e-6, nullptr, out5);
 }

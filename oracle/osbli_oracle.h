@@ -32,7 +32,7 @@ extern "C" {
 #endif
 
 enum { ORACLE_WENOZ5 = 0, ORACLE_TENO5 = 1, ORACLE_TENO6 = 2, ORACLE_WENOJS5 = 3, ORACLE_CENTRAL4 = 4,
-       ORACLE_WENOZ3 = 5 };
+       ORACLE_WENOZ3 = 5, ORACLE_WENOZ7 = 6 /* 7th-order WENO-Z, four ghost points */ };
 enum { ORACLE_VISC_NONE = 0, ORACLE_VISC_CONST = 1, ORACLE_VISC_SUTHERLAND = 2 };
 enum { ORACLE_BC_PERIODIC = 0, ORACLE_BC_EXTRAP0 = 1, ORACLE_BC_DIRICHLET = 2, ORACLE_BC_WALL_ISOTHERMAL = 3,
        ORACLE_BC_WALL_ADIABATIC = 4 };
@@ -78,6 +78,8 @@ double oracle_reconstruct6(double a, double b, double c, double d, double e, dou
                            double eps, double teno_ct, double *margin);
 
 /* beta_0 (R), beta_1 (C), beta_2 (L), beta_3 (4-point) and tau_6 of W6, for the pins. */
+/* WENO-7Z value at i+1/2 from v7 = nodes i-3..i+3; out5 (may be NULL) = beta_0..beta_3, tau_7 */
+double oracle_reconstruct7(const double *v7, double eps, double *out5);
 void oracle_teno6_indicators(double a, double b, double c, double d, double e, double f, double *out5);
 
 /* Roe-averaged eigensystem at an interface (step 2a-2b).  QL, QR: the two

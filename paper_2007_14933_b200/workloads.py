@@ -20,7 +20,7 @@ from typing import Optional
 
 import numpy as np
 
-WENOZ5, TENO5, TENO6, WENOJS5, CENTRAL4, WENOZ3 = 0, 1, 2, 3, 4, 5
+WENOZ5, TENO5, TENO6, WENOJS5, CENTRAL4, WENOZ3, WENOZ7 = 0, 1, 2, 3, 4, 5, 6
 VISC_NONE, VISC_CONST, VISC_SUTHERLAND = 0, 1, 2
 BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL, BC_WALL_ADIABATIC = 0, 1, 2, 3, 4
 AVG_ROE, AVG_SIMPLE = 0, 1
@@ -55,7 +55,7 @@ class Case:
 
     @property
     def halo(self):
-        return tuple(3 if v > 1 else 0 for v in self.n)
+        return halo_of(self.n, self.scheme)
 
     @property
     def periodic(self):
@@ -74,13 +74,15 @@ class Case:
 
 
 # ------------------------------------------------------------------------------ helpers ----
-def halo_of(n):
-    return tuple(3 if v > 1 else 0 for v in n)
+def halo_of(n, scheme=None):
+    """Ghost points per side: 3, 4 for the 7th-order scheme (stencil i-3..i+4); 0 in a collapsed direction."""
+    depth = 4 if scheme == WENOZ7 else 3
+    return tuple(depth if v > 1 else 0 for v in n)
 
 
-def padded_index_grids(n):
+def padded_index_grids(n, scheme=None):
     """Integer node indices (i, j, k) on the dense padded grid, as broadcastable arrays."""
-    h = halo_of(n)
+    h = halo_of(n, scheme)
     i = np.arange(-h[0], n[0] + h[0])[None, None, :]
     j = np.arange(-h[1], n[1] + h[1])[None, :, None]
     k = np.arange(-h[2], n[2] + h[2])[:, None, None]
@@ -100,9 +102,9 @@ def conservative(rho, u, v, w, p, gamma):
     return Q
 
 
-def edge_pad_interior(A, n):
+def edge_pad_interior(A, n, scheme=None):
     """Overwrite halo entries of dense padded array(s) [..., NZ, NY, NX] by an edge copy."""
-    h = halo_of(n)
+    h = halo_of(n, scheme)
     core = A[..., h[2]:h[2] + n[2], h[1]:h[1] + n[1], h[0]:h[0] + n[0]]
     pw = [(0, 0)] * (A.ndim - 3) + [(h[2],) * 2, (h[1],) * 2, (h[0],) * 2]
     return np.ascontiguousarray(np.pad(core, pw, mode="edge"))
@@ -121,13 +123,13 @@ def splitmix64_unit(seed, index):
 def sod(nx=400, scheme=WENOZ5, dt=2e-4, nsteps=1000):
     """1-D Sod shock tube (BASELINE.json config 1).  x_i = i/(nx-1)."""
     n = (nx, 1, 1)
-    i, _, _ = padded_index_grids(n)
+    i, _, _ = padded_index_grids(n, scheme)
     x = i / (nx - 1.0)
     left = x < 0.5
     rho = np.where(left, 1.0, 0.125)
     p = np.where(left, 1.0, 0.1)
     Q0 = conservative(rho, 0.0, 0.0, 0.0, p, 1.4)
-    Q0 = edge_pad_interior(Q0, n)
+    Q0 = edge_pad_interior(Q0, n, scheme)
     return Case(name=f"sod{nx}", n=n, Q0=Q0, dt=dt, nsteps=nsteps, delta=(1.0 / (nx - 1.0), 1.0, 1.0),
                 gamma=1.4, Minf=1.0, scheme=scheme, visc=VISC_NONE,
                 bc=((BC_EXTRAP0, BC_EXTRAP0), (0, 0), (0, 0)),
@@ -141,7 +143,7 @@ _TGV_DT = {64: (3.385e-3, 100), 256: (8.5e-4, 200), 512: (4.2e-4, 50)}
 def tgv(n=64, scheme=TENO5, visc=VISC_CONST, dt=None, nsteps=None, M=0.1, Re=1600.0, Pr=0.71):
     """3-D viscous Taylor-Green vortex on [0, 2 pi)^3 (BASELINE.json configs 2, 3, 5)."""
     nn = (n, n, n)
-    i, j, k = padded_index_grids(nn)
+    i, j, k = padded_index_grids(nn, scheme)
     h = 2.0 * np.pi / n
     x, y, z = i * h, j * h, k * h
     gamma = 1.4
@@ -166,7 +168,7 @@ def euler_wave(N=32, scheme=WENOZ5, A=0.04, dt=5e-4, t_end=2.5, curvilinear=True
     rho = 1 + 0.2 sin(pi (x + y - t (u + v))), u = 1, v = -0.5, p = 1; periodic, L_x = L_y = 2.
     """
     n = (N, N, 1)
-    i, j, k = padded_index_grids(n)
+    i, j, k = padded_index_grids(n, scheme)
     L = 2.0
     d = L / N
     x = i * d + A * np.sin(6.0 * np.pi * j * d / L) + 0.0 * k
@@ -183,7 +185,7 @@ def euler_wave(N=32, scheme=WENOZ5, A=0.04, dt=5e-4, t_end=2.5, curvilinear=True
     coords = np.ascontiguousarray(np.stack([x, y, np.zeros_like(x)])) if curvilinear else None
     per = (BC_PERIODIC, BC_PERIODIC)
     nsteps = int(round(t_end / dt))
-    h = halo_of(n)
+    h = halo_of(n, scheme)
     xi = x[:, h[1]:h[1] + N, h[0]:h[0] + N]
     yi = y[:, h[1]:h[1] + N, h[0]:h[0] + N]
     return Case(name=f"wave{N}", n=n, Q0=Q0, dt=dt, nsteps=nsteps, delta=(d, d, 1.0), coords=coords, gamma=gamma,
@@ -363,7 +365,7 @@ def wavy_box(n=(24, 20, 8), seed=1, bc=None, scheme=WENOZ5, visc=VISC_SUTHERLAND
         bc = ((BC_DIRICHLET, BC_EXTRAP0), (BC_WALL_ISOTHERMAL, BC_DIRICHLET), (BC_PERIODIC, BC_PERIODIC))
     per = tuple(bc[d][0] == BC_PERIODIC for d in range(3))
     rng = np.random.default_rng(seed)
-    i, j, k = padded_index_grids(n)
+    i, j, k = padded_index_grids(n, scheme)
     # computational coordinates in [0,1): periodic directions use n points per period, others n-1 intervals
     den = [float(n[d] if per[d] else max(n[d] - 1, 1)) for d in range(3)]
     xi, et, ze = i / den[0] + 0.0 * j + 0.0 * k, j / den[1] + 0.0 * i + 0.0 * k, k / den[2] + 0.0 * i + 0.0 * j
@@ -409,7 +411,7 @@ def perturb(case, seed=0, amp=0.02):
         ref = np.abs(Q[c][core]).max()
         scale = amp * (0.1 * ref if c in (0, 4) else max(ref, 0.1))
         Q[c][core] += scale * rng.uniform(-1.0, 1.0, size=Q[c][core].shape)
-    return edge_pad_interior(Q, case.n)
+    return edge_pad_interior(Q, case.n, case.scheme)
 
 
 def approximate_metrics(case):

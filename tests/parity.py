@@ -52,7 +52,7 @@ def report(**kw):
 def metrics_for(case):
     if case.coords is None:
         return None
-    return O.metrics_from_coords(case.coords, case.n, case.periodic, delta=case.delta)
+    return O.metrics_from_coords(case.coords, case.n, case.periodic, delta=case.delta, scheme=case.scheme)
 
 
 def make_oracle(case, metrics=None, **over):

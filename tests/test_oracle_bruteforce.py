@@ -7,7 +7,7 @@ a second time in a different shape: whole-array operations on periodically rolle
 eigenvector matrices applied with einsum, no loops over points.  It shares nothing with
 oracle/osbli_oracle.cpp (triple loops, one interface at a time) beyond the paper.
 
-Uniform grids, periodic boxes in 1-D, 2-D and 3-D, WENO-Z5 / TENO5 / TENO6 / WENO-JS5, mu = 1 viscous terms.
+Uniform grids, periodic boxes in 1-D, 2-D and 3-D, WENO-Z3/Z5/Z7 / TENO5 / TENO6 / WENO-JS5 / central, mu = 1 viscous terms.
 (Closures, wall and Dirichlet fills, Sutherland and metric terms are pinned on their own: P6, P11,
 P4/P8/P9, P10.)
 """
@@ -29,6 +29,24 @@ def prim(Q):
 
 def weights_and_value(pts, scheme, eps=1e-16, ct=1e-6):
     """pts: the stencil values [a, b, c, d, e(, f)], upwind side a, b, c; interface between c and d."""
+    if scheme == W.WENOZ7:
+        # k = 4: cubic candidates and the expanded indicators of the 7th-order scheme [18] (pts = nodes i-3..i+3),
+        # ideal weights (4, 18, 12, 1)/35 for candidates {i..i+3}, {i-1..i+2}, {i-2..i+1}, {i-3..i}; tau = |beta_0 - beta_3|
+        m3, m2, m1, c0, p1, p2, p3 = pts
+        q7 = [(3 * c0 + 13 * p1 - 5 * p2 + p3) / 12, (-m1 + 7 * c0 + 7 * p1 - p2) / 12,
+              (m2 - 5 * m1 + 13 * c0 + 3 * p1) / 12, (-3 * m3 + 13 * m2 - 23 * m1 + 25 * c0) / 12]
+        b7 = [(c0 * (2107 * c0 - 9402 * p1 + 7042 * p2 - 1854 * p3) + p1 * (11003 * p1 - 17246 * p2 + 4642 * p3)
+               + p2 * (7043 * p2 - 3882 * p3) + 547 * p3 ** 2) / 240,
+              (m1 * (547 * m1 - 2522 * c0 + 1922 * p1 - 494 * p2) + c0 * (3443 * c0 - 5966 * p1 + 1602 * p2)
+               + p1 * (2843 * p1 - 1642 * p2) + 267 * p2 ** 2) / 240,
+              (m2 * (267 * m2 - 1642 * m1 + 1602 * c0 - 494 * p1) + m1 * (2843 * m1 - 5966 * c0 + 1922 * p1)
+               + c0 * (3443 * c0 - 2522 * p1) + 547 * p1 ** 2) / 240,
+              (m3 * (547 * m3 - 3882 * m2 + 4642 * m1 - 1854 * c0) + m2 * (7043 * m2 - 17246 * m1 + 7042 * c0)
+               + m1 * (11003 * m1 - 9402 * c0) + 2107 * c0 ** 2) / 240]
+        t7 = np.abs(b7[0] - b7[3])
+        d7 = [4 / 35, 18 / 35, 12 / 35, 1 / 35]
+        al7 = [d7[r] * (1 + (t7 / (b7[r] + eps)) ** 2) for r in range(4)]
+        return sum(al7[r] * q7[r] for r in range(4)) / sum(al7)
     a, b, c, d, e = pts[:5]
     if scheme == W.WENOZ3:                                  # k = 2: two linear candidates, weights eq. (22)
         q3 = [(c + d) / 2, (-b + 3 * c) / 2]
@@ -103,13 +121,14 @@ def inviscid_sweep(Q, d, delta, scheme):
     H = (wl * Hn + wr * at(Hn, 1)) / (wl + wr)
     ar = np.sqrt((G - 1) * (H - 0.5 * (ut ** 2).sum(0)))
     L, R, _ = eigenvectors(ut, H, ar, n)
-    ms = list(range(-2, 4))
+    ms = list(range(-3, 5)) if scheme == W.WENOZ7 else list(range(-2, 4))
+    nw = len(ms)
     V = [np.einsum("...kc,c...->...k", L, at(Q, m)) for m in ms]    # [..., field] at stencil point m
     Gc = [np.einsum("...kc,c...->...k", L, at(F, m)) for m in ms]
     alpha = np.stack([np.max(np.stack([np.abs(at(lam[k], m)) for m in ms]), 0) for k in range(5)], -1)
-    gp = [0.5 * (Gc[j] + alpha * V[j]) for j in range(6)]
-    gm = [0.5 * (Gc[j] - alpha * V[j]) for j in range(6)]
-    npts = 6 if scheme == W.TENO6 else 5
+    gp = [0.5 * (Gc[j] + alpha * V[j]) for j in range(nw)]
+    gm = [0.5 * (Gc[j] - alpha * V[j]) for j in range(nw)]
+    npts = 7 if scheme == W.WENOZ7 else (6 if scheme == W.TENO6 else 5)
     ghat = weights_and_value(gp[:npts], scheme) + weights_and_value(gm[::-1][:npts], scheme)
     fhat = np.einsum("...ck,...k->c...", R, ghat)                   # f^_{i+1/2}, component first
     return -(fhat - np.roll(fhat, 1, axis=ax)) / delta
@@ -169,9 +188,9 @@ def brute_residual(case, scheme, visc):
     return R
 
 
-def box(n, seed):
+def box(n, seed, scheme=None):
     rng = np.random.default_rng(seed)
-    i, j, k = W.padded_index_grids(n)
+    i, j, k = W.padded_index_grids(n, scheme)
     x, y, z = 2 * np.pi * i / n[0], 2 * np.pi * j / n[1], 2 * np.pi * k / n[2]
     ph = rng.uniform(0, 2 * np.pi, 8)
     rho = 1.0 + 0.3 * np.sin(x + ph[0]) * np.cos(y + ph[1]) + 0.1 * np.cos(z + ph[2])
@@ -184,14 +203,15 @@ def box(n, seed):
     per = (W.BC_PERIODIC, W.BC_PERIODIC)
     bc = tuple(per if n[d] > 1 else (0, 0) for d in range(3))
     return W.Case(name="brute", n=n, Q0=np.ascontiguousarray(W.conservative(rho, u, v, w, p, G)), dt=1e-3, nsteps=1,
-                  delta=tuple(2 * np.pi / v_ for v_ in n), gamma=G, Re=50.0, Pr=0.71, Minf=0.7, bc=bc)
+                  delta=tuple(2 * np.pi / v_ for v_ in n), gamma=G, Re=50.0, Pr=0.71, Minf=0.7, bc=bc,
+                  **({} if scheme is None else {"scheme": scheme}))
 
 
-@pytest.mark.parametrize("scheme", [W.WENOZ5, W.TENO5, W.TENO6, W.WENOJS5, W.CENTRAL4, W.WENOZ3])
+@pytest.mark.parametrize("scheme", [W.WENOZ5, W.TENO5, W.TENO6, W.WENOJS5, W.CENTRAL4, W.WENOZ3, W.WENOZ7])
 @pytest.mark.parametrize("n", [(8, 6, 5), (12, 10, 1), (16, 1, 1)])
 @pytest.mark.parametrize("visc", [W.VISC_NONE, W.VISC_CONST])
 def test_p12_oracle_equals_vectorised_numpy(scheme, n, visc):
-    case = box(n, seed=sum(n) + scheme)
+    case = box(n, seed=sum(n) + scheme, scheme=scheme if scheme == W.WENOZ7 else None)      # the 7th-order scheme: halo 4
     orc = O.Oracle(**{**case.physics(), "scheme": scheme, "visc": visc, "eps": 1e-6 if scheme == W.WENOJS5 else 1e-16})
     Ro = orc.interior(orc.rhs(orc.bc(case.Q0.copy())))
     Rb = brute_residual(case, scheme, visc != W.VISC_NONE)
