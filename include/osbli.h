@@ -28,7 +28,7 @@
  * Node (i,j,k) of variable c, with i in [-halo[0], nx+halo[0]) etc., lives at
  *     c*stride_var + (k+halo[2])*stride_z + (j+halo[1])*stride_y + x_offset + i        (doubles)
  * halo[d] = 3 for an active direction (n_d > 1; "ghost points required by the
- * shock-capturing schemes"), 0 for an inactive one (n_d == 1: no halo, no sweep).  x_offset and
+ * shock-capturing schemes"; 4 with OSBLI_SCHEME_WENOZ7, stencil i-3..i+4), 0 for an inactive one (n_d == 1: no halo, no sweep).  x_offset and
  * stride_y are multiples of 16 doubles so that interior node i = 0 of every row is 128-byte
  * aligned when the base pointer is.  Metric fields and the Dirichlet state use the same layout
  * (one field / five fields).  Entries that are neither interior nor halo are never read.
@@ -48,7 +48,9 @@ enum { OSBLI_OK = 0, OSBLI_EINVAL = 1, OSBLI_EUNSUPPORTED = 2, OSBLI_ECUDA = 3, 
 enum { OSBLI_SCHEME_WENOZ5 = 0, OSBLI_SCHEME_TENO5 = 1, OSBLI_SCHEME_TENO6 = 2,
        OSBLI_SCHEME_WENOJS5 = 3 /* eq. (20)-(21); set eps = 1e-6 */,
        OSBLI_SCHEME_CENTRAL4 = 4 /* eq. (28) on the flux vectors, no shock capturing; uniform grids */,
-       OSBLI_SCHEME_WENOZ3 = 5 /* third-order WENO-Z */ };
+       OSBLI_SCHEME_WENOZ3 = 5 /* third-order WENO-Z */,
+       OSBLI_SCHEME_WENOZ7 = 6 /* seventh-order WENO-Z: halo 4, untuned sweeps,
+                                  separate stage update */ };
 enum { OSBLI_VISC_NONE = 0 /* Euler */, OSBLI_VISC_CONST = 1 /* mu = 1 */,
        OSBLI_VISC_SUTHERLAND = 2 /* PAPER.md:59-63, 317-318 */ };
 enum { OSBLI_BC_PERIODIC = 0, OSBLI_BC_EXTRAP0 = 1, OSBLI_BC_DIRICHLET = 2,
@@ -116,7 +118,7 @@ int osbli_workspace_bytes(const osbli_params *p, size_t *out);
  * direction are ignored), OSBLI_ECUDA (no sm_100 device / runtime failure). */
 int osbli_init(const osbli_params *p, void *d_workspace, size_t workspace_bytes, osbli_handle *out);
 
-/* Fill the 3-deep halos (and, for DIRICHLET / WALL, the boundary plane) of device state Q in
+/* Fill the halos (depth layout.halo) (and, for DIRICHLET / WALL, the boundary plane) of device state Q in
  * place: x, then y over the x-extended range, then z over the x,y-extended range, so edges and
  * corners are defined.  PERIODIC: wrap.  EXTRAP0: zero-order extrapolation of the boundary
  * node.  DIRICHLET: boundary plane + halos copied from params.dirichlet

@@ -12,7 +12,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libosbli.so"
-SOURCES = ["osbli_sweep.cu", "osbli_api.cu", "osbli_visc.cu", "osbli_central.cu", "osbli_bc_rk.cu", "osbli_peak.cu"]
+SOURCES = ["osbli_sweep.cu", "osbli_weno7.cu", "osbli_api.cu", "osbli_visc.cu", "osbli_central.cu", "osbli_bc_rk.cu", "osbli_peak.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -35,7 +35,7 @@ int make_layout(const osbli_params *p, Layout *L) {
     if (n[d] < 1) return OSBLI_EINVAL;
     if (n[d] > 1 && n[d] < 5) return OSBLI_EINVAL;
     L->n[d] = n[d];
-    L->h[d] = n[d] > 1 ? kHalo : 0;
+    L->h[d] = n[d] > 1 ? (p->scheme == OSBLI_SCHEME_WENOZ7 ? kHalo7 : kHalo) : 0;
   }
   L->xoff = kXOffset;
   const long long rowlen = kXOffset + (long long)n[0] + kXTail;
@@ -61,7 +61,7 @@ int validate(const osbli_params *p) {
   Layout L;
   if (int rc = make_layout(p, &L)) return rc;
   if (p->nx == 1) return OSBLI_EUNSUPPORTED;                       // x is the contiguous direction; it must be active
-  if (p->scheme < OSBLI_SCHEME_WENOZ5 || p->scheme > OSBLI_SCHEME_WENOZ3) return OSBLI_EINVAL;
+  if (p->scheme < OSBLI_SCHEME_WENOZ5 || p->scheme > OSBLI_SCHEME_WENOZ7) return OSBLI_EINVAL;
   if (p->scheme == OSBLI_SCHEME_CENTRAL4 && p->metrics) return OSBLI_EUNSUPPORTED;   // central convective terms: uniform grids
   if (p->visc < OSBLI_VISC_NONE || p->visc > OSBLI_VISC_SUTHERLAND) return OSBLI_EINVAL;
   if (p->averaging != OSBLI_AVG_ROE && p->averaging != OSBLI_AVG_SIMPLE) return OSBLI_EINVAL;
@@ -157,7 +157,11 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
       }
       if (P.has_force) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_force(P, Q, R, st));
     }
-    OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep(P, d, Q, R, accumulate, d == last ? rk : nullptr, st));
+    if (P.scheme == OSBLI_SCHEME_WENOZ7) {                          // side scheme: its own untuned sweeps, no fused update
+      if (rk) return OSBLI_EINVAL;
+      OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep7(P, d, Q, R, accumulate, st));
+    } else
+      OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep(P, d, Q, R, accumulate, d == last ? rk : nullptr, st));
     accumulate = 1;
   }
   if (last == 0 && P.visc != OSBLI_VISC_NONE)                       // 1-D: the x sweep, then the viscous terms
@@ -189,7 +193,8 @@ int do_step(osbli_ctx *h, int nstages, double *Q, double *Qtmp, double dt, cudaS
     }
     return OSBLI_OK;
   }
-  const bool fuse = (h->P.L.n[1] > 1 || h->P.L.n[2] > 1) && h->P.scheme != OSBLI_SCHEME_CENTRAL4;
+  const bool fuse = (h->P.L.n[1] > 1 || h->P.L.n[2] > 1) && h->P.scheme != OSBLI_SCHEME_CENTRAL4 &&
+                    h->P.scheme != OSBLI_SCHEME_WENOZ7;
   bool wrap = fuse;                  // every active direction periodic: the fused update fills the halos itself
   for (int d = 0; d < 3; ++d)
     if (h->P.L.n[d] > 1 && !h->P.periodic[d]) wrap = false;

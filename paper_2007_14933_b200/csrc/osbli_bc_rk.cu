@@ -24,6 +24,7 @@ bc_kernel(const __grid_constant__ DevParams P, double *__restrict__ Q) {
   const long long s = L.stride(DIR);
   const long long sv = L.sv;
   const int n = L.n[DIR];
+  const int hd = L.h[DIR];                         // halo depth: 3, or 4 for the 7th-order scheme
 
 #pragma unroll
   for (int side = 0; side < 2; ++side) {
@@ -31,7 +32,7 @@ bc_kernel(const __grid_constant__ DevParams P, double *__restrict__ Q) {
     const long long wall = base + (side == 0 ? 0 : (long long)(n - 1) * s);   // boundary node
     const long long inw = side == 0 ? s : -s;                                   // one node into the domain
     if (type == 0) {                   // periodic wrap
-      for (int m = 1; m <= 3; ++m)
+      for (int m = 1; m <= hd; ++m)
         for (int c = 0; c < 5; ++c) {
           double *q = Q + c * sv;
           if (side == 0) q[base - m * s] = q[base + (long long)(n - m) * s];
@@ -40,10 +41,10 @@ bc_kernel(const __grid_constant__ DevParams P, double *__restrict__ Q) {
     } else if (type == 1) {            // zero-order extrapolation
       for (int c = 0; c < 5; ++c) {
         const double v = Q[c * sv + wall];
-        for (int m = 1; m <= 3; ++m) Q[c * sv + wall - m * inw] = v;
+        for (int m = 1; m <= hd; ++m) Q[c * sv + wall - m * inw] = v;
       }
     } else if (type == 2) {            // Dirichlet: boundary plane and halos from the frozen state
-      for (int m = 0; m <= 3; ++m)
+      for (int m = 0; m <= hd; ++m)
         for (int c = 0; c < 5; ++c) Q[c * sv + wall - m * inw] = __ldg(P.dirichlet + c * sv + wall - m * inw);
     } else {                           // no-slip wall, eq. (40)-(46): isothermal (3) or adiabatic (4)
       auto temperature = [&](long long a) {
@@ -68,7 +69,7 @@ bc_kernel(const __grid_constant__ DevParams P, double *__restrict__ Q) {
         const double p = P.gm1 * (E - 0.5 * r * (u * u + v * v + w * w));
         T1 = P.gM2 * p / r;
       }
-      for (int m = 1; m <= 3; ++m) {
+      for (int m = 1; m <= hd; ++m) {
         const double Tm = (m + 1) * Tw - m * T1;             // eq. (42)
         const double rm = P.gM2 * pw / Tm;                   // eq. (43)
         const long long a = wall + m * inw, g = wall - m * inw;

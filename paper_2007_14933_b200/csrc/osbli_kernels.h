@@ -16,6 +16,9 @@ void rk_coefficients(int nstages, int form, int stage, double *A, double *B);   
 cudaError_t launch_sweep(const DevParams &P, int dir, const double *Q, double *R, int accumulate, const RkArgs *rk,
                          cudaStream_t st);
 
+// 7th-order WENO-Z sweeps (scheme 6, osbli_weno7.cu): R (-)= flux difference along `dir`; no fused update
+cudaError_t launch_sweep7(const DevParams &P, int dir, const double *Q, double *R, int accumulate, cudaStream_t st);
+
 // staged primitive fields u, v, w, T (, mu) on the halo-extended grid, then R += viscous terms (osbli_visc.cu)
 cudaError_t launch_primitives(const DevParams &P, const double *Q, double *prim, cudaStream_t st);
 cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *prim, double *R, int accumulate, cudaStream_t st);

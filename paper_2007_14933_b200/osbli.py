@@ -8,7 +8,7 @@ Functions carry the C names (`osbli_get_layout`, `osbli_workspace_bytes`, `osbli
 `osbli_destroy`, `osbli_strerror`); `Solver` bundles a handle with its torch-owned buffers.
 
 Dense <-> padded conversion (`to_padded`, `from_padded`) is pure data movement between the
-exchange format of `workloads.py` ([.., NZ, NY, NX] with halo 3) and the library's padded,
+exchange format of `workloads.py` ([.., NZ, NY, NX] with halo 3; 4 for the 7th-order scheme) and the library's padded,
 128-byte-aligned rows.
 """
 from __future__ import annotations
@@ -25,7 +25,7 @@ if not _LIBPATH.exists():
 _lib = C.CDLL(str(_LIBPATH))
 
 OK, EINVAL, EUNSUPPORTED, ECUDA, EWORKSPACE = 0, 1, 2, 3, 4
-SCHEME_WENOZ5, SCHEME_TENO5, SCHEME_TENO6, SCHEME_WENOJS5, SCHEME_CENTRAL4, SCHEME_WENOZ3 = 0, 1, 2, 3, 4, 5
+SCHEME_WENOZ5, SCHEME_TENO5, SCHEME_TENO6, SCHEME_WENOJS5, SCHEME_CENTRAL4, SCHEME_WENOZ3, SCHEME_WENOZ7 = 0, 1, 2, 3, 4, 5, 6
 VISC_NONE, VISC_CONST, VISC_SUTHERLAND = 0, 1, 2
 BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL, BC_WALL_ADIABATIC = 0, 1, 2, 3, 4
 AVG_ROE, AVG_SIMPLE = 0, 1

@@ -136,6 +136,25 @@ def sod(nx=400, scheme=WENOZ5, dt=2e-4, nsteps=1000):
                 extra={"x": np.arange(nx) / (nx - 1.0), "t_end": dt * nsteps})
 
 
+def shu_osher(nx=320, scheme=WENOZ5, dt=2e-4, nsteps=9000):
+    """1-D shock / density-wave interaction: x in [-5, 5], Dirichlet ends, t_end = 1.8.
+
+    Left of x = -4 the post-shock state (3.857143, 2.629369, 10.33333); right of it rho = 1 + 0.2 sin(5x) at rest
+    with p = 1 (the printed "(.., 1.0, 0.0)" has u and p swapped: p = 0 is not a state; Q41)."""
+    n = (nx, 1, 1)
+    i, _, _ = padded_index_grids(n, scheme)
+    x = -5.0 + 10.0 * i / (nx - 1.0)
+    left = x < -4.0
+    rho = np.where(left, 3.857143, 1.0 + 0.2 * np.sin(5.0 * x))
+    u = np.where(left, 2.629369, 0.0)
+    p = np.where(left, 10.33333, 1.0)
+    Q0 = np.ascontiguousarray(conservative(rho, u, 0.0, 0.0, p, 1.4))
+    return Case(name=f"shu_osher{nx}", n=n, Q0=Q0, dt=dt, nsteps=nsteps, delta=(10.0 / (nx - 1.0), 1.0, 1.0),
+                gamma=1.4, Minf=1.0, scheme=scheme, visc=VISC_NONE,
+                bc=((BC_DIRICHLET, BC_DIRICHLET), (0, 0), (0, 0)), dirichlet=Q0.copy(),
+                extra={"x": -5.0 + 10.0 * np.arange(nx) / (nx - 1.0), "t_end": dt * nsteps})
+
+
 # ----------------------------------------------------------------------------- C2/C3/C5 ----
 _TGV_DT = {64: (3.385e-3, 100), 256: (8.5e-4, 200), 512: (4.2e-4, 50)}
 

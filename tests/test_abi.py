@@ -59,6 +59,9 @@ def test_layout_alignment_and_sizes(osbli):
         assert lay.stride_z == lay.stride_y * (n[1] + 2 * halo[1])
         assert lay.stride_var == lay.stride_z * (n[2] + 2 * halo[2])
         assert lay.total_doubles == 5 * lay.stride_var
+    lay = osbli.osbli_get_layout(osbli.make_params(n=(70, 37, 1), scheme=osbli.SCHEME_WENOZ7))      # 7th order: four ghost points
+    assert list(lay.halo) == [4, 4, 0] and lay.stride_y >= lay.x_offset + 70 + 4 and lay.x_offset >= 4
+    assert lay.stride_var == lay.stride_y * (37 + 8)
     p = osbli.make_params(n=(512, 512, 512), visc=osbli.VISC_CONST)
     lay = osbli.osbli_get_layout(p)
     assert 5.3e9 < lay.total_doubles * 8 < 6.2e9                          # "about 5.4 GB per state" + halos

@@ -178,7 +178,7 @@ def test_steps_curvilinear_walls():
 
 def _periodic_box(n, M=0.4, Re=100.0, scheme=W.TENO5, visc=W.VISC_CONST, bc=None, dt=2e-3):
     """Smooth periodic field on an n[0] x n[1] x n[2] box (n_d = 1: inactive direction)."""
-    i, j, k = W.padded_index_grids(n)
+    i, j, k = W.padded_index_grids(n, scheme)
     x, y, z = 2 * np.pi * i / n[0], 2 * np.pi * j / n[1], 2 * np.pi * k / n[2]
     g = 1.4
     u = np.sin(x) * np.cos(y) * np.cos(z)
@@ -295,6 +295,30 @@ def test_wenoz3_scheme():
     run_residual_case("sod_t0.03_wenoz3", sod, Q0=orc.run(sod.Q0.copy(), sod.dt, 150))
     run_steps_case("tgv32_10_wenoz3", case, 10, 1e-9, parity.q28)
     run_steps_case("sod_300_wenoz3", sod, 300, 1e-9, parity.l1_rel)
+
+
+def test_wenoz7_scheme():
+    """seventh-order WENO-Z (scheme 6; halo depth 4, eight-point window, its own sweeps and
+    the separate stage update): periodic 3-D with and without viscous terms, ragged sizes, a 2-D problem, the
+    curvilinear walled box (Dirichlet / wall / extrapolation fills four deep, Sutherland), 1-D shocks."""
+    case = W.tgv(32, scheme=W.WENOZ7)
+    assert case.halo == (4, 4, 4)
+    run_residual_case("tgv32_wenoz7", case)
+    run_residual_case("tgv32_wenoz7_perturbed", case, Q0=W.perturb(case, seed=5, amp=0.05))
+    run_residual_case("pbox_wenoz7_ragged", _periodic_box((37, 21, 13), scheme=W.WENOZ7))
+    run_residual_case("pbox2d_wenoz7_euler", _periodic_box((40, 33, 1), scheme=W.WENOZ7, visc=W.VISC_NONE))
+    run_residual_case("wavy_box_wenoz7", W.wavy_box(n=(40, 21, 9), scheme=W.WENOZ7))
+    run_residual_case("wave32_wenoz7", W.euler_wave(32, scheme=W.WENOZ7))
+    sod = W.sod(scheme=W.WENOZ7)
+    orc = parity.make_oracle(sod)
+    run_residual_case("sod_t0.03_wenoz7", sod, Q0=orc.run(sod.Q0.copy(), sod.dt, 150))
+    so = W.shu_osher(scheme=W.WENOZ7)
+    run_residual_case("shu_osher_t0_wenoz7", so)
+    run_steps_case("tgv32_10_wenoz7", case, 10, 1e-9, parity.q28)
+    run_steps_case("pbox_wenoz7_ragged_3", _periodic_box((37, 21, 13), scheme=W.WENOZ7), 3, 1e-9, parity.q28)
+    run_steps_case("wavy_box_wenoz7_3", W.wavy_box(n=(40, 21, 9), scheme=W.WENOZ7), 3, 1e-9, parity.l1_rel)
+    run_steps_case("sod_300_wenoz7", sod, 300, 1e-9, parity.l1_rel)
+    run_steps_case("shu_osher_500_wenoz7", so, 500, 1e-9, parity.l1_rel)
 
 
 def test_advance_host_matches_device_steps():
