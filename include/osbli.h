@@ -10,6 +10,7 @@
  *                     + 4th-order central viscous / heat flux      45-57 (eq. 1-5), 198-228 (eq. 28-35)
  *   - osbli_rk3_step  3-stage low-storage Runge-Kutta step         PAPER.md:232-242 (eq. 36-38)
  *   - osbli_rk4_step  5-stage 4th-order member of the same family
+ *   - osbli_rk3_step_static  osbli_rk3_step without a handle or a caller workspace (static scratch, <= 64 MiB)
  *   - osbli_advance_host  same, from/to HOST memory (copies inside)
  *
  * Conventions
@@ -44,7 +45,8 @@ extern "C" {
 
 typedef struct osbli_ctx *osbli_handle;
 
-enum { OSBLI_OK = 0, OSBLI_EINVAL = 1, OSBLI_EUNSUPPORTED = 2, OSBLI_ECUDA = 3, OSBLI_EWORKSPACE = 4 };
+enum { OSBLI_OK = 0, OSBLI_EINVAL = 1, OSBLI_EUNSUPPORTED = 2, OSBLI_ECUDA = 3, OSBLI_EWORKSPACE = 4,
+       OSBLI_ESTATIC = 5 /* osbli_rk3_step_static only: the problem exceeds OSBLI_STATIC_SCRATCH_BYTES */ };
 enum { OSBLI_SCHEME_WENOZ5 = 0, OSBLI_SCHEME_TENO5 = 1, OSBLI_SCHEME_TENO6 = 2,
        OSBLI_SCHEME_WENOJS5 = 3 /* eq. (20)-(21); set eps = 1e-6 */,
        OSBLI_SCHEME_CENTRAL4 = 4 /* eq. (28) on the flux vectors, no shock capturing; uniform grids */,
@@ -147,6 +149,25 @@ int osbli_rk3_step(osbli_handle h, double *d_Q, double *d_Qtmp, double dt, void 
 /* The same with the five-stage 4th-order member of the family eq. (36)-(38) ("The 3rd and
  * 4th order schemes have three and five sub-stages per iteration"): Q -> Q2 -> Q3 -> Q2 -> Q3 -> Q. */
 int osbli_rk4_step(osbli_handle h, double *d_Q, double *d_Qtmp, double dt, void *cuda_stream);
+
+/* osbli_rk3_step for callers that cannot allocate device memory or keep a handle (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): the same RK3 step (eq. (36)-(38), same kernels, same
+ * order, same result as osbli_init + osbli_rk3_step), with the workspace (R, Q2, Q3, staged primitives) in a
+ * file-scope static device array of OSBLI_STATIC_SCRATCH_BYTES inside the library instead of a caller-provided one.
+ * The call allocates nothing on the host or the device (no cudaMalloc / cudaFree, no handle); every device that
+ * loads the library holds the array until the process exits.
+ *   p        host pointer; read during the call only.  p->dirichlet / p->metrics: device pointers as for osbli_init.
+ *   d_Q      device pointer, state in the padded layout of osbli_get_layout(p): advanced in place, halos filled.
+ *   d_Qtmp   device pointer, dU accumulator (overwritten, need not be initialised); both stay owned by the caller.
+ * Limit: osbli_workspace_bytes(p) <= OSBLI_STATIC_SCRATCH_BYTES (64 MiB: e.g. the 1-D cases, 64^3 with the fast
+ * viscous path, 48^3 with the general one); beyond it the call returns OSBLI_ESTATIC and launches nothing.  Other
+ * errors as osbli_init.  All calls on a device share the one array, which keeps the last call's contents (the part
+ * a call uses is cleared on the stream first): calls that may overlap on the GPU (different streams, or threads)
+ * race and must be serialised by the caller.  The per-device set-up (array address, shared-memory attributes)
+ * happens on the first call on each device, with that device current. */
+#define OSBLI_STATIC_SCRATCH_BYTES ((size_t)64 << 20)
+size_t osbli_static_scratch_bytes(void);
+int osbli_rk3_step_static(const osbli_params *p, double *d_Q, double *d_Qtmp, double dt, void *cuda_stream);
 
 /* End-to-end convenience with HOST buffers: copies the interior nodes of h_Q (host, padded layout,
  * total_doubles doubles) to d_Q, runs nsteps RK3 steps of size dt (halos are rebuilt on the device),

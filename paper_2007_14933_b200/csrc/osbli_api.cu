@@ -1,6 +1,7 @@
 // osbli_api.cu -- host side of the C ABI declared in include/osbli.h: layout, parameter
 // validation, launch sequencing on the caller's stream.  No device allocation, no synchronisation
 // (except osbli_advance_host), no CPU fallback.
+#include <mutex>
 #include "../../include/osbli.h"
 #include "osbli_kernels.h"
 
@@ -217,6 +218,48 @@ int do_step(osbli_ctx *h, int nstages, double *Q, double *Qtmp, double dt, cudaS
   return wrap ? OSBLI_OK : do_bc(h, Q, st);
 }
 
+// A context from validated parameters and a workspace of osbli_workspace_bytes(p) bytes (no allocation; the
+// profiling list is the caller's business).
+void fill_ctx(const osbli_params *p, void *d_workspace, osbli_ctx *h) {
+  std::memset(h, 0, sizeof(*h));
+  DevParams &P = h->P;
+  make_layout(p, &P.L);
+  P.curvilinear = p->metrics ? 1 : 0;
+  const double dl[3] = {p->dx, p->dy, p->dz};
+  for (int d = 0; d < 3; ++d) {
+    const double delta = (P.L.n[d] > 1 && !P.curvilinear) ? dl[d] : 1.0;
+    P.inv_delta[d] = 1.0 / delta;
+    P.inv12d[d] = 1.0 / (12.0 * delta);
+    P.inv12d2[d] = 1.0 / (12.0 * delta * delta);
+    P.periodic[d] = p->bc[d][0] == OSBLI_BC_PERIODIC;
+    for (int s = 0; s < 2; ++s) { P.bc[d][s] = p->bc[d][s]; P.wall_T[d][s] = p->wall_T[d][s]; }
+  }
+  P.gamma = p->gamma; P.gm1 = p->gamma - 1.0;
+  P.Re = p->Re; P.inv_Re = p->visc != OSBLI_VISC_NONE ? 1.0 / p->Re : 0.0;
+  P.Pr = p->Pr; P.Minf = p->Minf; P.gM2 = p->gamma * p->Minf * p->Minf;
+  P.cq = p->visc != OSBLI_VISC_NONE ? 1.0 / ((p->gamma - 1.0) * p->Minf * p->Minf * p->Pr * p->Re) : 0.0;
+  P.scheme = p->scheme; P.visc = p->visc;
+  P.ct = p->teno_ct; P.eps = p->eps; P.suth = p->suth_ratio;
+  const double nstencils = p->scheme == OSBLI_SCHEME_TENO6 ? 4.0 : 3.0;
+  P.teno_kfast = (std::pow(nstencils * p->teno_ct, -1.0 / 6.0) - 1.0) * (1.0 - 1e-6);
+  P.dirichlet = p->dirichlet;
+  for (int a = 0; a < 3; ++a) P.force[a] = p->force[a];
+  P.has_force = (p->force[0] != 0.0 || p->force[1] != 0.0 || p->force[2] != 0.0) ? 1 : 0;
+  P.averaging = p->averaging;
+  P.rk3_form = p->rk3_form;
+  if (p->metrics) {
+    for (int k = 0; k < 3; ++k) {
+      for (int j = 0; j < 3; ++j) P.D[k][j] = p->metrics->D[k][j];
+      for (int e = 0; e < 6; ++e) P.E[k][e] = p->metrics->E[k][e];
+    }
+    P.detJ = p->metrics->detJ;
+  }
+  h->R = static_cast<double *>(d_workspace);
+  h->Q2 = h->R + 5 * P.L.sv;
+  h->Q3 = h->Q2 + 5 * P.L.sv;
+  h->prim = h->Q3 + 5 * P.L.sv;
+}
+
 }  // namespace
 
 extern "C" {
@@ -260,45 +303,9 @@ int osbli_init(const osbli_params *p, void *d_workspace, size_t workspace_bytes,
 
   osbli_ctx *h = new (std::nothrow) osbli_ctx;
   if (!h) return OSBLI_EINVAL;
-  std::memset(h, 0, sizeof(*h));
-  DevParams &P = h->P;
-  make_layout(p, &P.L);
-  P.curvilinear = p->metrics ? 1 : 0;
-  const double dl[3] = {p->dx, p->dy, p->dz};
-  for (int d = 0; d < 3; ++d) {
-    const double delta = (P.L.n[d] > 1 && !P.curvilinear) ? dl[d] : 1.0;
-    P.inv_delta[d] = 1.0 / delta;
-    P.inv12d[d] = 1.0 / (12.0 * delta);
-    P.inv12d2[d] = 1.0 / (12.0 * delta * delta);
-    P.periodic[d] = p->bc[d][0] == OSBLI_BC_PERIODIC;
-    for (int s = 0; s < 2; ++s) { P.bc[d][s] = p->bc[d][s]; P.wall_T[d][s] = p->wall_T[d][s]; }
-  }
-  P.gamma = p->gamma; P.gm1 = p->gamma - 1.0;
-  P.Re = p->Re; P.inv_Re = p->visc != OSBLI_VISC_NONE ? 1.0 / p->Re : 0.0;
-  P.Pr = p->Pr; P.Minf = p->Minf; P.gM2 = p->gamma * p->Minf * p->Minf;
-  P.cq = p->visc != OSBLI_VISC_NONE ? 1.0 / ((p->gamma - 1.0) * p->Minf * p->Minf * p->Pr * p->Re) : 0.0;
-  P.scheme = p->scheme; P.visc = p->visc;
-  P.ct = p->teno_ct; P.eps = p->eps; P.suth = p->suth_ratio;
-  const double nstencils = p->scheme == OSBLI_SCHEME_TENO6 ? 4.0 : 3.0;
-  P.teno_kfast = (std::pow(nstencils * p->teno_ct, -1.0 / 6.0) - 1.0) * (1.0 - 1e-6);
-  P.dirichlet = p->dirichlet;
-  for (int a = 0; a < 3; ++a) P.force[a] = p->force[a];
-  P.has_force = (p->force[0] != 0.0 || p->force[1] != 0.0 || p->force[2] != 0.0) ? 1 : 0;
-  P.averaging = p->averaging;
-  P.rk3_form = p->rk3_form;
-  if (p->metrics) {
-    for (int k = 0; k < 3; ++k) {
-      for (int j = 0; j < 3; ++j) P.D[k][j] = p->metrics->D[k][j];
-      for (int e = 0; e < 6; ++e) P.E[k][e] = p->metrics->E[k][e];
-    }
-    P.detJ = p->metrics->detJ;
-  }
+  fill_ctx(p, d_workspace, h);
   h->prof = new (std::nothrow) std::vector<ProfiledLaunch>();
   if (!h->prof) { delete h; return OSBLI_EINVAL; }
-  h->R = static_cast<double *>(d_workspace);
-  h->Q2 = h->R + 5 * P.L.sv;
-  h->Q3 = h->Q2 + 5 * P.L.sv;
-  h->prim = h->Q3 + 5 * P.L.sv;
   *out = h;
   return OSBLI_OK;
 }
@@ -456,6 +463,58 @@ int osbli_destroy(osbli_handle h) {
   return OSBLI_OK;
 }
 
+// ---- osbli_rk3_step_static: one RK3 step with the workspace in a static device array (include/osbli.h) ----------
+// Every device that loads the library holds these OSBLI_STATIC_SCRATCH_BYTES until the process exits.  In host code
+// the name g_static_scratch is a host-side stand-in, not a device address: the address a kernel can use comes from
+// cudaGetSymbolAddress, once per device, with that device current (static_scratch_setup).
+}  // extern "C"
+
+static __device__ __align__(256) double g_static_scratch[OSBLI_STATIC_SCRATCH_BYTES / sizeof(double)];
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mu;
+double *g_static_ptr[kMaxDevices];     // device address of g_static_scratch on each device ordinal (nullptr: not set up)
+
+// Once per device, with that device current: opt-in shared-memory sizes of the kernels and the array's device address.
+int static_scratch_setup(int dev, double **out) {
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_ptr[dev]) {
+    int major = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess || major != 10) return OSBLI_ECUDA;
+    if (sweep_set_attributes() != cudaSuccess || viscous_set_attributes() != cudaSuccess || central_set_attributes() != cudaSuccess) return OSBLI_ECUDA;
+    double *ptr = nullptr;
+    if (cudaGetSymbolAddress(reinterpret_cast<void **>(&ptr), g_static_scratch) != cudaSuccess || !ptr) return OSBLI_ECUDA;
+    if (reinterpret_cast<uintptr_t>(ptr) & 255u) return OSBLI_ECUDA;
+    g_static_ptr[dev] = ptr;
+  }
+  *out = g_static_ptr[dev];
+  return OSBLI_OK;
+}
+}  // namespace
+
+extern "C" {
+
+size_t osbli_static_scratch_bytes(void) { return OSBLI_STATIC_SCRATCH_BYTES; }
+
+int osbli_rk3_step_static(const osbli_params *p, double *d_Q, double *d_Qtmp, double dt, void *cuda_stream) {
+  if (!d_Q || !d_Qtmp || d_Q == d_Qtmp) return OSBLI_EINVAL;
+  if (int rc = validate(p)) return rc;
+  size_t need = 0;
+  if (int rc = osbli_workspace_bytes(p, &need)) return rc;
+  if (need > OSBLI_STATIC_SCRATCH_BYTES) return OSBLI_ESTATIC;     // the problem does not fit the static array
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return OSBLI_ECUDA;
+  double *ws = nullptr;
+  if (int rc = static_scratch_setup(dev, &ws)) return rc;
+  cudaStream_t st = as_stream(cuda_stream);
+  // the array keeps the last call's contents (possibly of another problem shape): start from zeros
+  if (cudaMemsetAsync(ws, 0, need, st) != cudaSuccess) return OSBLI_ECUDA;
+  osbli_ctx ctx;                                                    // on the stack: no handle, nothing to free
+  fill_ctx(p, ws, &ctx);
+  return do_step(&ctx, 3, d_Q, d_Qtmp, dt, st);
+}
+
 const char *osbli_strerror(int status) {
   switch (status) {
     case OSBLI_OK: return "ok";
@@ -463,6 +522,7 @@ const char *osbli_strerror(int status) {
     case OSBLI_EUNSUPPORTED: return "unsupported configuration";
     case OSBLI_ECUDA: return "CUDA error (no sm_100 device, or a launch / copy failed)";
     case OSBLI_EWORKSPACE: return "workspace missing, too small or not 256-byte aligned";
+    case OSBLI_ESTATIC: return "problem too large for osbli_rk3_step_static: its workspace exceeds OSBLI_STATIC_SCRATCH_BYTES (64 MiB)";
     default: return "unknown status";
   }
 }

@@ -24,7 +24,7 @@ if not _LIBPATH.exists():
                       "(there is no CPU fallback for the osbli hot path)")
 _lib = C.CDLL(str(_LIBPATH))
 
-OK, EINVAL, EUNSUPPORTED, ECUDA, EWORKSPACE = 0, 1, 2, 3, 4
+OK, EINVAL, EUNSUPPORTED, ECUDA, EWORKSPACE, ESTATIC = 0, 1, 2, 3, 4, 5
 SCHEME_WENOZ5, SCHEME_TENO5, SCHEME_TENO6, SCHEME_WENOJS5, SCHEME_CENTRAL4, SCHEME_WENOZ3, SCHEME_WENOZ7 = 0, 1, 2, 3, 4, 5, 6
 VISC_NONE, VISC_CONST, VISC_SUTHERLAND = 0, 1, 2
 BC_PERIODIC, BC_EXTRAP0, BC_DIRICHLET, BC_WALL_ISOTHERMAL, BC_WALL_ADIABATIC = 0, 1, 2, 3, 4
@@ -75,6 +75,10 @@ _lib.osbli_rhs.restype = C.c_int
 _lib.osbli_rhs.argtypes = [_h, _dp, _dp, _dp]
 _lib.osbli_rk3_step.restype = C.c_int
 _lib.osbli_rk3_step.argtypes = [_h, _dp, _dp, C.c_double, _dp]
+_lib.osbli_static_scratch_bytes.restype = C.c_size_t
+_lib.osbli_static_scratch_bytes.argtypes = []
+_lib.osbli_rk3_step_static.restype = C.c_int
+_lib.osbli_rk3_step_static.argtypes = [C.POINTER(Params), _dp, _dp, C.c_double, _dp]
 _lib.osbli_rk4_step.restype = C.c_int
 _lib.osbli_rk4_step.argtypes = [_h, _dp, _dp, C.c_double, _dp]
 _lib.osbli_advance_host.restype = C.c_int
@@ -95,7 +99,7 @@ _lib.osbli_strerror.restype = C.c_char_p
 _lib.osbli_strerror.argtypes = [C.c_int]
 
 EXPORTS = ("osbli_get_layout", "osbli_workspace_bytes", "osbli_init", "osbli_bc", "osbli_rhs",
-           "osbli_rk3_step", "osbli_rk4_step", "osbli_advance_host", "osbli_advance_host_batch", "osbli_launch_count", "osbli_profile_begin", "osbli_profile_end",
+           "osbli_rk3_step", "osbli_rk3_step_static", "osbli_static_scratch_bytes", "osbli_rk4_step", "osbli_advance_host", "osbli_advance_host_batch", "osbli_launch_count", "osbli_profile_begin", "osbli_profile_end",
            "osbli_measure_fp64_peak", "osbli_destroy", "osbli_strerror")
 K_CLASSES = ("bc", "primitives", "sweep_x", "sweep_y", "sweep_z", "viscous", "rk_update")
 
@@ -144,6 +148,15 @@ def osbli_rhs(handle, q_ptr, r_ptr, stream=0):
 
 def osbli_rk3_step(handle, q_ptr, qtmp_ptr, dt, stream=0):
     _check(_lib.osbli_rk3_step(handle, q_ptr, qtmp_ptr, float(dt), stream), "osbli_rk3_step")
+
+
+def osbli_static_scratch_bytes() -> int:
+    return int(_lib.osbli_static_scratch_bytes())
+
+
+def osbli_rk3_step_static(params: Params, q_ptr, qtmp_ptr, dt, stream=0):
+    """One RK3 step with the workspace in the library's static device array: no handle, no allocation (osbli.h)."""
+    _check(_lib.osbli_rk3_step_static(C.byref(params), q_ptr, qtmp_ptr, float(dt), stream), "osbli_rk3_step_static")
 
 
 def osbli_rk4_step(handle, q_ptr, qtmp_ptr, dt, stream=0):
