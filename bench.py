@@ -39,7 +39,8 @@ FLOP_SWEEP = {0: 1256 + 15 + 19, 1: 1356 + 15 + 19,      # WENO-Z5, TENO5: inter
               2: 1856 + 15 + 19,                          # TENO6: + ~50 per reconstruction (hand count)
               3: 1206 + 15 + 19,                          # WENO-JS5: WENO-Z5 minus tau and the (1 + (.)^2) factors
               4: 90,                                      # central4: 4 stencil points x ~17 flop + combination, per direction
-              5: 900}                                     # WENO-Z3: projections as for the 5-point schemes, ~25 per reconstruction
+              5: 900,                                     # WENO-Z3: projections as for the 5-point schemes, ~25 per reconstruction
+              6: 2300}                                    # WENO-Z7: 8-point projections, ~110 per reconstruction (hand count)
 FLOP_VISCOUS = 300
 FLOP_RK = 20
 # Curvilinear grids (config 4): SURVEY.md 8(d) estimates "metric products add ~25 %" and 5500 flop per point-stage
@@ -53,7 +54,7 @@ def make_case(args):
     """The workload: (case, metrics or None, label, BASELINE.json config number or None)."""
     from paper_2007_14933_b200 import workloads as W
     schemes = {"wenoz5": W.WENOZ5, "teno5": W.TENO5, "teno6": W.TENO6, "wenojs5": W.WENOJS5,
-               "central4": W.CENTRAL4, "wenoz3": W.WENOZ3}
+               "central4": W.CENTRAL4, "wenoz3": W.WENOZ3, "wenoz7": W.WENOZ7}
     if args.config == 4:
         case = W.sbli_slab()
         label = ("SBLI slab 500x250x8 curvilinear, WENO-Z5 + central-4 viscous (Sutherland), isothermal wall / Dirichlet / "
@@ -198,7 +199,7 @@ def cpu_sample_case(args, full=False):
         return W.sbli_slab(n=n), f"the same slab (grid, flow, boundaries) on {n[0]}x{n[1]}x{n[2]} points"
     big = 512 if args.config == 5 else args.n
     n = min(big, 256) if full else 64
-    schemes = {"wenoz5": W.WENOZ5, "teno5": W.TENO5, "teno6": W.TENO6, "wenojs5": W.WENOJS5, "central4": W.CENTRAL4, "wenoz3": W.WENOZ3}
+    schemes = {"wenoz5": W.WENOZ5, "teno5": W.TENO5, "teno6": W.TENO6, "wenojs5": W.WENOJS5, "central4": W.CENTRAL4, "wenoz3": W.WENOZ3, "wenoz7": W.WENOZ7}
     case = W.tgv(n, scheme=schemes[args.scheme])
     if case.scheme == W.WENOJS5:
         case.eps = 1e-6
@@ -466,7 +467,7 @@ def main():
     ap.add_argument("--perturb", type=float, default=0.0,
                     help="side measurement: seeded perturbation amplitude of the TGV state (non-smooth data takes the full TENO evaluation)")
     ap.add_argument("--n", type=int, default=256, help="grid points per side of the TGV (256 = BASELINE.json config 3)")
-    ap.add_argument("--scheme", default="teno5", choices=["wenoz5", "teno5", "teno6", "wenojs5", "central4", "wenoz3"],
+    ap.add_argument("--scheme", default="teno5", choices=["wenoz5", "teno5", "teno6", "wenojs5", "central4", "wenoz3", "wenoz7"],
                     help="reconstruction (teno5 = BASELINE.json config 3; the others are side measurements)")
     args = ap.parse_args()
     if args.impl == "reference":
