@@ -25,6 +25,9 @@ namespace osbli {
 #ifndef OSBLI_X_MINB
 #define OSBLI_X_MINB 1
 #endif
+#ifndef OSBLI_PREPOINT
+#define OSBLI_PREPOINT 0      // y/z sweeps on uniform grids: the point entering the window is prepared one interface ahead
+#endif
 // RK = 0: R (-)= flux difference.  RK = 1 / 2: this is the last kernel of the stage and also does
 // the low-storage Runge-Kutta update eq. (36)-(37) of its nodes (1: first stage, A_0 = 0, dU is not
 // read): with R_in the residual accumulated by the earlier kernels of the stage,
@@ -127,6 +130,16 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
   issue_rd(s0);
   if constexpr (kAsyncQ) issue_q(s0 + 3);
   else load(s0 + 2, qn, Kn);                     // prefetched raw state of the next node
+  // kPre: the thermodynamics of the entering point (a serial chain: rsqrt -> velocities -> p -> a) is not the first
+  // thing an interface waits for but runs one interface ahead, next to the reconstruction of the previous one:
+  // wn = point q+3 of interface q, made during interface q-1 from the raw state loaded one more node ahead.
+  constexpr bool kPre = OSBLI_PREPOINT && !CURV && !kAsyncQ;
+  Pt<CURV> wn;
+  double rsn = 1.0;
+  if constexpr (kPre) {
+    make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], wn, rsn);   // node s0+2
+    load(min(s0 + 3, s1 + 2), qn, Kn);
+  }
 
   for (int q = s0 - 1; q < s1; ++q) {            // interface q+1/2, between nodes q and q+1
 #pragma unroll
@@ -137,9 +150,15 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
 #pragma unroll
       for (int c = 0; c < 5; ++c) qn[c] = stg[6 + ((q + 3) & 1)][c][threadIdx.x];
     }
-    make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], w[5], rsq[2]);
+    if constexpr (kPre) {
+      w[5] = wn; rsq[2] = rsn;
+      make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], wn, rsn);   // node q+4 (clamped)
+      load(min(q + 5, s1 + 2), qn, Kn);          // unconditional (clamped to the last node any interface reads)
+    } else {
+      make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], w[5], rsq[2]);
+    }
     if constexpr (CURV) { KR.advance(); KR.put(5, Kn[0], Kn[1], Kn[2]); }
-    if constexpr (!kAsyncQ) {
+    if constexpr (!kAsyncQ && !kPre) {
       if (q + 1 < s1) load(q + 4, qn, Kn);       // node (q+1)+3, used by the next interface
     }
     issue_rd(q + 2);
