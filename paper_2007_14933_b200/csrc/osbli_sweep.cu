@@ -25,18 +25,6 @@ namespace osbli {
 #ifndef OSBLI_X_MINB
 #define OSBLI_X_MINB 1
 #endif
-#ifndef OSBLI_PREPOINT
-#define OSBLI_PREPOINT 0      // y/z sweeps on uniform grids: the point entering the window is prepared one interface ahead
-#endif
-#ifndef OSBLI_PREPOINT_RK
-#define OSBLI_PREPOINT_RK 0   // the same in the sweep fused with the stage update (raw states staged three deep)
-#endif
-#ifndef OSBLI_PREAVG
-#define OSBLI_PREAVG 0        // uniform grids: the interface average (step 2(a)) is formed one interface ahead as well
-#endif
-#ifndef OSBLI_PREPOINT_X
-#define OSBLI_PREPOINT_X 0    // the same in the x sweep
-#endif
 // RK = 0: R (-)= flux difference.  RK = 1 / 2: this is the last kernel of the stage and also does
 // the low-storage Runge-Kutta update eq. (36)-(37) of its nodes (1: first stage, A_0 = 0, dU is not
 // read): with R_in the residual accumulated by the earlier kernels of the stage,
@@ -49,8 +37,7 @@ __global__ void __launch_bounds__(128, CURV ? 1 : OSBLI_YZ_MINB)
 sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R,
                 int chunk, const RkArgs rk) {
   static_assert(DIR == 1 || DIR == 2, "x has its own kernel");
-  constexpr bool kPreRK = OSBLI_PREPOINT_RK && !CURV && RK != 0;      // raw states staged three deep (slots 6-8, node % 3)
-  __shared__ double stg[CURV ? 6 : (kPreRK ? 9 : 8)][5][128];   // per-thread slots: R (0-2) and dU (3-5) of nodes n % 3, raw state (6-7) of nodes n & 1
+  __shared__ double stg[CURV ? 6 : 8][5][128];   // per-thread slots: R (0-2) and dU (3-5) of nodes n % 3, raw state (6-7) of nodes n & 1
   __shared__ double kring[CURV ? 18 : 1][128];    // curvilinear: K_m of the six window points (KRing)
   KRing<128> KR{&kring[0][threadIdx.x], 0};
   const Layout &Ly = P.L;
@@ -109,13 +96,6 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
   // flight for HBM with 8 warps per SM): R (and dU) of node n travel by cp.async into the per-thread slot n % 3,
   // issued while interface n-2 is computed; in the fused update on uniform grids the raw state of the node that
   // enters the window is staged the same way (slot n & 1), elsewhere it is prefetched into registers.
-  constexpr bool kPreAvg = OSBLI_PREAVG && !CURV;
-  IfaceAvg An;                                   // kPreAvg: average of the interface the next iteration computes
-  if constexpr (kPreAvg) {
-    const RoeSide r4 = roe_side<CURV>(P, w[4], rsq[1]);          // node s0
-    An = iface_avg(P, rl, r4);
-    rl = r4;
-  }
   constexpr bool kAsyncQ = !CURV && RK != 0;
   constexpr int kGroups = kAsyncQ ? 2 : 1;       // cp.async groups committed per iteration
   auto issue_rd = [&](int node) {                // group 1: R, dU of `node` (empty outside [s0, s1))
@@ -136,66 +116,40 @@ sweep_yz_kernel(const __grid_constant__ DevParams P, const double *__restrict__ 
     if (node <= s1 + 2) {
       const long long o = line0 + (long long)node * st;
 #pragma unroll
-      for (int c = 0; c < 5; ++c) cp_async8(&stg[6 + (kPreRK ? node % 3 : (node & 1))][c][threadIdx.x], Q + c * sv + o);
+      for (int c = 0; c < 5; ++c) cp_async8(&stg[6 + (node & 1)][c][threadIdx.x], Q + c * sv + o);
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
   };
   double qn[5], Kn[3] = {0.0, 0.0, 0.0};
   // prologue = what iterations s0-3 and s0-2 would have issued
-  if constexpr (kPreRK) load(s0 + 2, qn, Kn);    // the first entering point is made in front of the loop: plain load
   issue_rd(s0 - 1);
-  if constexpr (kAsyncQ) issue_q(s0 + (kPreRK ? 3 : 2));
+  if constexpr (kAsyncQ) issue_q(s0 + 2);
   issue_rd(s0);
-  if constexpr (kAsyncQ) issue_q(s0 + (kPreRK ? 4 : 3));
+  if constexpr (kAsyncQ) issue_q(s0 + 3);
   else load(s0 + 2, qn, Kn);                     // prefetched raw state of the next node
-  // kPre: the thermodynamics of the entering point (a serial chain: rsqrt -> velocities -> p -> a) is not the first
-  // thing an interface waits for but runs one interface ahead, next to the reconstruction of the previous one:
-  // wn = point q+3 of interface q, made during interface q-1 from the raw state loaded one more node ahead.
-  constexpr bool kPre = OSBLI_PREPOINT && !CURV && !kAsyncQ;
-  Pt<CURV> wn;
-  double rsn = 1.0;
-  if constexpr (kPre || kPreRK) {
-    make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], wn, rsn);   // node s0+2
-    if constexpr (kPre) load(min(s0 + 3, s1 + 2), qn, Kn);
-  }
 
   for (int q = s0 - 1; q < s1; ++q) {            // interface q+1/2, between nodes q and q+1
 #pragma unroll
     for (int m = 0; m < 5; ++m) w[m] = w[m + 1];
     rsq[0] = rsq[1]; rsq[1] = rsq[2];
     if constexpr (kAsyncQ) {
-      asm volatile("cp.async.wait_group 2;" ::: "memory");      // node q+3 (kPreRK: q+4) has landed (issued two iterations ago)
+      asm volatile("cp.async.wait_group 2;" ::: "memory");      // node q+3 has landed (issued two iterations ago)
 #pragma unroll
-      for (int c = 0; c < 5; ++c) qn[c] = stg[6 + (kPreRK ? (q + 4) % 3 : ((q + 3) & 1))][c][threadIdx.x];
+      for (int c = 0; c < 5; ++c) qn[c] = stg[6 + ((q + 3) & 1)][c][threadIdx.x];
     }
-    if constexpr (kPre || kPreRK) {
-      w[5] = wn; rsq[2] = rsn;
-      // node q+4 (kPre: clamped; kPreRK: past s1+2 nothing was staged and the point made of the slot's old contents is never used)
-      make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], wn, rsn);
-      if constexpr (kPre) load(min(q + 5, s1 + 2), qn, Kn);     // unconditional (clamped to the last node any interface reads)
-    } else {
-      make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], w[5], rsq[2]);
-    }
+    make_point<DIR, CURV>(P, qn[0], qn[1], qn[2], qn[3], qn[4], Kn[0], Kn[1], Kn[2], w[5], rsq[2]);
     if constexpr (CURV) { KR.advance(); KR.put(5, Kn[0], Kn[1], Kn[2]); }
-    if constexpr (!kAsyncQ && !kPre) {
+    if constexpr (!kAsyncQ) {
       if (q + 1 < s1) load(q + 4, qn, Kn);       // node (q+1)+3, used by the next interface
     }
     issue_rd(q + 2);
-    if constexpr (kAsyncQ) issue_q(q + (kPreRK ? 6 : 5));
+    if constexpr (kAsyncQ) issue_q(q + 5);
     double rold[5] = {0, 0, 0, 0, 0};
+    const RoeSide rr = roe_side<CURV>(P, w[3], rsq[0]);
     double f[5];
-    if constexpr (kPreAvg) {
-      const IfaceAvg A = An;
-      const RoeSide r4 = roe_side<CURV>(P, w[4], rsq[1]);        // node q+2: the average of interface q+1 does not wait
-      An = iface_avg(P, rl, r4);
-      rl = r4;
-      interface_flux_avg<DIR, SCHEME>(w, A, rp, f);
-    } else {
-      const RoeSide rr = roe_side<CURV>(P, w[3], rsq[0]);
-      if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, KR, rl, rr, rp, f);
-      else interface_flux<DIR, SCHEME>(P, w, rl, rr, rp, f);
-      rl = rr;
-    }
+    if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, KR, rl, rr, rp, f);
+    else interface_flux<DIR, SCHEME>(P, w, rl, rr, rp, f);
+    rl = rr;
     if (q >= s0) {
       const long long o = line0 + (long long)q * st;
       double sc = inv_d;
@@ -340,20 +294,14 @@ sweep_x_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q
   load_tile(a_in);
   __syncwarp();
 
-  // kPreX: the point made in iteration `node` enters the window one iteration later, so that its thermodynamics
-  // (a serial chain) runs next to the reconstruction of interface node-4 instead of in front of interface node-3.
-  constexpr bool kPreX = OSBLI_PREPOINT_X && !CURV;
-  Pt<CURV> wn = w[5];
-  double rsn = 1.0;
-  IfaceAvg An = {{0.0, 0.0, 0.0}, 0.0, 1.0, 1.0, 1.0, 1.0};       // OSBLI_PREAVG: average of the interface the next iteration computes
-  for (int node = s0 - 3; node < s1 + 3 + (kPreX ? 1 : 0); ++node) {   // node entering window slot 5 (kPreX: being prepared)
-    if (node >= a_in + kXT && (!kPreX || node < s1 + 3)) {
+  for (int node = s0 - 3; node < s1 + 3; ++node) {               // node entering window slot 5
+    if (node >= a_in + kXT) {
       __syncwarp();
       a_in += kXT;
       load_tile(a_in);
       __syncwarp();
     }
-    const int col = node - a_in;                                 // kPreX, last iteration: may be the pad column (never used)
+    const int col = node - a_in;
 #pragma unroll
     for (int m = 0; m < 5; ++m) w[m] = w[m + 1];
     rsq[0] = rsq[1]; rsq[1] = rsq[2];
@@ -367,38 +315,17 @@ sweep_x_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q
         kx = J * S.in[6][lane][col]; ky = J * S.in[7][lane][col]; kz = J * S.in[8][lane][col];
         Jw[3] = J;
       }
-      if constexpr (kPreX) {
-        w[5] = wn; rsq[2] = rsn;
-        make_point<0, CURV>(P, r, mx, my, mz, E, kx, ky, kz, wn, rsn);
-      } else {
-        make_point<0, CURV>(P, r, mx, my, mz, E, kx, ky, kz, w[5], rsq[2]);
-      }
+      make_point<0, CURV>(P, r, mx, my, mz, E, kx, ky, kz, w[5], rsq[2]);
       if constexpr (CURV) { KR.advance(); KR.put(5, kx, ky, kz); }
     }
-    const int q = node - (kPreX ? 4 : 3);                        // interface q+1/2 is now computable
-    constexpr bool kPreAvg = OSBLI_PREAVG && !CURV;
-    if (q == s0 - 2) {
-      rl = roe_side<CURV>(P, w[3], rsq[0]);                        // slot 3 holds node s0-1
-      if constexpr (kPreAvg) {
-        const RoeSide r4 = roe_side<CURV>(P, w[4], rsq[1]);        // node s0
-        An = iface_avg(P, rl, r4);
-        rl = r4;
-      }
-    }
+    const int q = node - 3;                                      // interface q+1/2 is now computable
+    if (q == s0 - 2) rl = roe_side<CURV>(P, w[3], rsq[0]);         // slot 3 holds node s0-1
     if (q < s0 - 1) continue;
+    const RoeSide rr = roe_side<CURV>(P, w[3], rsq[0]);
     double f[5];
-    if constexpr (kPreAvg) {
-      const IfaceAvg A = An;
-      const RoeSide r4 = roe_side<CURV>(P, w[4], rsq[1]);          // node q+2
-      An = iface_avg(P, rl, r4);
-      rl = r4;
-      interface_flux_avg<0, SCHEME>(w, A, rp, f);
-    } else {
-      const RoeSide rr = roe_side<CURV>(P, w[3], rsq[0]);
-      if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, KR, rl, rr, rp, f);
-      else interface_flux<0, SCHEME>(P, w, rl, rr, rp, f);
-      rl = rr;
-    }
+    if constexpr (CURV) interface_flux_curv<SCHEME>(P, w, KR, rl, rr, rp, f);
+    else interface_flux<0, SCHEME>(P, w, rl, rr, rp, f);
+    rl = rr;
     if (q >= s0) {
       double sc = inv_d;
       if constexpr (CURV) sc = 1.0 / Jw[0];                      // slot 2 = node q
