@@ -2,12 +2,13 @@
 // (22); used at 7th order in PAPER.md:485-495 and 531-533; Q40): R (-)= (f^_{i+1/2} - f^_{i-1/2}) / Delta_d
 // (or / detJ_i) with the characteristic flux reconstruction of PAPER.md:100-111 on the eight-point window i-3..i+4.
 //
-// A side scheme, written for correctness and not tuned like the 5th/6th-order sweeps of
-// osbli_sweep.cu: one thread per node evaluates both of its interface fluxes (each interface twice over the grid),
-// eigenvectors are applied as dense 5x5 matrices for a general unit normal (uniform grids: e_d), the stage update is
-// the separate rk_update_kernel.  What it shares with the tuned path is the layout, the boundary fills and the
-// viscous kernels; the halo depth is 4 (Layout::h).
+// A side scheme: a tiled kernel of its own (below), not the register-window march of the
+// 5th/6th-order sweeps (an 8-point window of staged points does not fit the register file next to the rest); dense
+// eigenvectors for a general unit normal (uniform grids: e_d), the stage update is the separate rk_update_kernel.  What
+// it shares with the tuned path is the layout, the boundary fills and the viscous kernels; halo depth 4 (Layout::h).
 #include "osbli_kernels.h"
+
+#include <type_traits>
 
 namespace osbli {
 
@@ -54,129 +55,213 @@ __device__ __forceinline__ double weno7z(const double (&v)[7], double eps) {
   return v[3] + num / den;
 }
 
-// f^_{i+1/2} between node `at` and `at + s` (s = stride of DIR), PAPER.md:100-111 steps 1-2.
-template <int DIR, bool CURV>
-__device__ __forceinline__ void interface_flux7(const DevParams &P, const double *__restrict__ Q, long long at, long long s,
-                                                double (&fhat)[5]) {
-  const long long sv = P.L.sv;
-  double U[8][5], F[8][5], lam[8][3], Kil[2][3];
-  // step 1: solution vector, flux and wave speeds at the eight stencil points i-3..i+4
-#pragma unroll
-  for (int m = 0; m < 8; ++m) {
-    const long long pt = at + (long long)(m - 3) * s;
-#pragma unroll
-    for (int c = 0; c < 5; ++c) U[m][c] = __ldg(Q + c * sv + pt);
-    double K[3] = {DIR == 0 ? 1.0 : 0.0, DIR == 1 ? 1.0 : 0.0, DIR == 2 ? 1.0 : 0.0};
-    if constexpr (CURV) {
-      const double J = __ldg(P.detJ + pt);
-#pragma unroll
-      for (int a = 0; a < 3; ++a) K[a] = J * __ldg(P.D[DIR][a] + pt);
-    }
-    if (m == 3 || m == 4) { Kil[m - 3][0] = K[0]; Kil[m - 3][1] = K[1]; Kil[m - 3][2] = K[2]; }
-    const double ir = 1.0 / U[m][0];
-    const double u = U[m][1] * ir, v = U[m][2] * ir, w = U[m][3] * ir;
-    const double p = P.gm1 * (U[m][4] - 0.5 * (U[m][1] * u + U[m][2] * v + U[m][3] * w));
-    const double a = sqrt(P.gamma * p * ir);
-    const double th = K[0] * u + K[1] * v + K[2] * w;
-    const double Kn = CURV ? sqrt(K[0] * K[0] + K[1] * K[1] + K[2] * K[2]) : 1.0;
-    F[m][0] = U[m][0] * th;
-    F[m][1] = fma(U[m][1], th, p * K[0]);
-    F[m][2] = fma(U[m][2], th, p * K[1]);
-    F[m][3] = fma(U[m][3], th, p * K[2]);
-    F[m][4] = (U[m][4] + p) * th;
-    lam[m][0] = fabs(th); lam[m][1] = fabs(th + a * Kn); lam[m][2] = fabs(th - a * Kn);
-  }
-  // step 2(a): Roe (or simple) average of nodes i, i+1; interface normal from the averaged K
-  double n[3] = {DIR == 0 ? 1.0 : 0.0, DIR == 1 ? 1.0 : 0.0, DIR == 2 ? 1.0 : 0.0};
-  if constexpr (CURV) {
-    const double kx = 0.5 * (Kil[0][0] + Kil[1][0]), ky = 0.5 * (Kil[0][1] + Kil[1][1]), kz = 0.5 * (Kil[0][2] + Kil[1][2]);
-    const double ik = 1.0 / sqrt(kx * kx + ky * ky + kz * kz);
-    n[0] = kx * ik; n[1] = ky * ik; n[2] = kz * ik;
-  }
-  double u, v, w, H;
-  {
-    const double *UL = U[3], *UR = U[4];
-    if (P.averaging != 0) {            // U_{i+1/2} = (U_i + U_{i+1})/2
-      const double r = 0.5 * (UL[0] + UR[0]), ir = 1.0 / r;
-      u = 0.5 * (UL[1] + UR[1]) * ir; v = 0.5 * (UL[2] + UR[2]) * ir; w = 0.5 * (UL[3] + UR[3]) * ir;
-      const double E = 0.5 * (UL[4] + UR[4]);
-      const double p = P.gm1 * (E - 0.5 * r * (u * u + v * v + w * w));
-      H = (E + p) * ir;
-    } else {
-      const double pL = P.gm1 * (UL[4] - 0.5 * (UL[1] * UL[1] + UL[2] * UL[2] + UL[3] * UL[3]) / UL[0]);
-      const double pR = P.gm1 * (UR[4] - 0.5 * (UR[1] * UR[1] + UR[2] * UR[2] + UR[3] * UR[3]) / UR[0]);
-      const double sl = sqrt(UL[0]), sr = sqrt(UR[0]), is = 1.0 / (sl + sr);
-      u = (UL[1] / sl + UR[1] / sr) * is; v = (UL[2] / sl + UR[2] / sr) * is; w = (UL[3] / sl + UR[3] / sr) * is;
-      H = ((UL[4] + pL) / sl + (UR[4] + pR) / sr) * is;
-    }
-  }
-  const double q2 = u * u + v * v + w * w;
-  const double a = sqrt(P.gm1 * (H - 0.5 * q2));
-  const double th = n[0] * u + n[1] * v + n[2] * w;
-  const double b1 = P.gm1 / (a * a), b2 = 0.5 * b1 * q2;
-  // step 2(b): left eigenvectors (rows) and right eigenvectors for the unit normal n: fields 0, 1, 2
-  // (speed theta): l_k = n_k (1 - b2, b1 u, -b1) + ((m - rho u~) x n)_k; fields 3, 4: theta +- a
-  const double Lm[5][5] = {
-      {n[0] * (1.0 - b2) - (v * n[2] - w * n[1]), n[0] * b1 * u, n[0] * b1 * v + n[2], n[0] * b1 * w - n[1], -n[0] * b1},
-      {n[1] * (1.0 - b2) - (w * n[0] - u * n[2]), n[1] * b1 * u - n[2], n[1] * b1 * v, n[1] * b1 * w + n[0], -n[1] * b1},
-      {n[2] * (1.0 - b2) - (u * n[1] - v * n[0]), n[2] * b1 * u + n[1], n[2] * b1 * v - n[0], n[2] * b1 * w, -n[2] * b1},
-      {0.5 * (b2 - th / a), 0.5 * (-b1 * u + n[0] / a), 0.5 * (-b1 * v + n[1] / a), 0.5 * (-b1 * w + n[2] / a), 0.5 * b1},
-      {0.5 * (b2 + th / a), 0.5 * (-b1 * u - n[0] / a), 0.5 * (-b1 * v - n[1] / a), 0.5 * (-b1 * w - n[2] / a), 0.5 * b1}};
-  const double Rm[5][5] = {   // Rm[k][c]: component c of r_k
-      {n[0], u * n[0], v * n[0] + n[2], w * n[0] - n[1], 0.5 * q2 * n[0] + v * n[2] - w * n[1]},
-      {n[1], u * n[1] - n[2], v * n[1], w * n[1] + n[0], 0.5 * q2 * n[1] + w * n[0] - u * n[2]},
-      {n[2], u * n[2] + n[1], v * n[2] - n[0], w * n[2], 0.5 * q2 * n[2] + u * n[1] - v * n[0]},
-      {1.0, u + a * n[0], v + a * n[1], w + a * n[2], H + a * th},
-      {1.0, u - a * n[0], v - a * n[1], w - a * n[2], H - a * th}};
-#pragma unroll
-  for (int c = 0; c < 5; ++c) fhat[c] = 0.0;
-#pragma unroll
-  for (int k = 0; k < 5; ++k) {
-    const int lk = k < 3 ? 0 : (k == 3 ? 1 : 2);
-    double alpha = 0.0;                                  // step 2(d): max over the stencil points (Q10)
-#pragma unroll
-    for (int m = 0; m < 8; ++m) alpha = fmax(alpha, lam[m][lk]);
-    double gp[8], gm[8];
-#pragma unroll
-    for (int m = 0; m < 8; ++m) {                        // step 2(c), eq. (13)
-      double V = 0.0, G = 0.0;
-#pragma unroll
-      for (int c = 0; c < 5; ++c) { V = fma(Lm[k][c], U[m][c], V); G = fma(Lm[k][c], F[m][c], G); }
-      gp[m] = 0.5 * fma(alpha, V, G);
-      gm[m] = 0.5 * fma(-alpha, V, G);
-    }
-    const double vp[7] = {gp[0], gp[1], gp[2], gp[3], gp[4], gp[5], gp[6]};
-    const double vm[7] = {gm[7], gm[6], gm[5], gm[4], gm[3], gm[2], gm[1]};       // mirror image (Q4)
-    const double gk = weno7z(vp, P.eps) + weno7z(vm, P.eps);                       // step 2(e)
-#pragma unroll
-    for (int c = 0; c < 5; ++c) fhat[c] = fma(gk, Rm[k][c], fhat[c]);              // step 2(f)
-  }
-}
+// ---------------------------------------------------------------------------------------------
+// Tiled kernel.  A block owns NS consecutive nodes of 32 (y, z sweeps: x-neighbouring) or 8 (x sweep) grid lines
+// along the sweep direction.  (1) The NS + 8 stencil points of every line are staged once in shared memory as
+// (U, p, theta = K.u, c = a |K| [, K]); (2) thread (f, line) computes the ONE interface flux between nodes s0-1+f and
+// s0+f, f = 0..NS (PAPER.md:100-111 steps 2(a)-(f)), reading the staged points field by field, and leaves it in shared
+// memory; (3) thread (f < NS, line) takes the difference (step 3, eq. (10)) for node s0+f.  Every point's
+// thermodynamics is computed (NS+8)/NS times and every flux (NS+1)/NS times.
+//   y, z sweeps: threadIdx.x = x lane (coalesced rows), threadIdx.y = f;  NS = 8 (6 on curvilinear grids: 3 more
+//   staged doubles per point);   x sweep: threadIdx.x = f (32 interfaces, NS = 31 nodes), threadIdx.y = line of 8.
+template <int DIR, bool CURV> struct Tile7 {
+  static constexpr int NS = DIR == 0 ? 31 : (CURV ? 6 : 8);      // nodes per block along the sweep
+  static constexpr int NF = NS + 1, NP = NS + 8;                  // interfaces, staged points (s0-4 .. s0+NS+3)
+  static constexpr int NT = DIR == 0 ? 8 : 32;                    // lines per block
+  static constexpr int NV = CURV ? 11 : 8;                        // staged doubles per point
+  static constexpr int NTHREADS = NF * NT;
+  // (p, t) -> index; the fastest index is the one consecutive lanes differ in (no bank conflicts)
+  static __device__ __forceinline__ int at(int p, int t) { return DIR == 0 ? t * NP + p : p * NT + t; }
+  static __device__ __forceinline__ int fat(int f, int t) { return DIR == 0 ? t * NF + f : f * NT + t; }
+};
 
 template <int DIR, bool CURV>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__((Tile7<DIR, CURV>::NTHREADS), 2)
 sweep7_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R, int accumulate) {
+  using T7 = Tile7<DIR, CURV>;
+  constexpr int NS = T7::NS, NF = T7::NF, NP = T7::NP, NT = T7::NT, NV = T7::NV;
+  __shared__ double pts[NV][NP * NT];
+  __shared__ double flx[5][NF * NT];
   const Layout &L = P.L;
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= L.n[0]) return;
-  const long long at = L.at(i, blockIdx.y, blockIdx.z), s = L.stride(DIR), sv = L.sv;
-  double fr[5], fl[5];
-  interface_flux7<DIR, CURV>(P, Q, at, s, fr);
-  interface_flux7<DIR, CURV>(P, Q, at - s, s, fl);
-  double sc = P.inv_delta[DIR];
-  if constexpr (CURV) sc = 1.0 / __ldg(P.detJ + at);
+  const long long sv = L.sv, st = L.stride(DIR);
+  const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+  const int f = DIR == 0 ? threadIdx.x : threadIdx.y;             // interface between nodes s0-1+f and s0+f
+  const int t = DIR == 0 ? threadIdx.y : threadIdx.x;             // line within the block
+  const int n = L.n[DIR];
+  int s0;
+  // node 0 of line t (clamped to the last valid line: its results are computed and not stored)
+  auto line_base = [&](int tt, bool &valid) -> long long {
+    if constexpr (DIR == 0) {
+      const int nl = L.n[1] * L.n[2];
+      int line = blockIdx.y * NT + tt;
+      valid = line < nl;
+      line = min(line, nl - 1);
+      return L.at(0, line % L.n[1], line / L.n[1]);
+    } else {
+      int i = blockIdx.x * NT + tt;
+      valid = i < L.n[0];
+      i = min(i, L.n[0] - 1);
+      return DIR == 1 ? L.at(i, 0, blockIdx.y) : L.at(i, blockIdx.y, 0);
+    }
+  };
+  if constexpr (DIR == 0) s0 = blockIdx.x * NS; else s0 = blockIdx.z * NS;
+
+  // (1) stage the points
+  for (int e = tid; e < NP * NT; e += T7::NTHREADS) {
+    const int pp = DIR == 0 ? e % NP : e / NT, tt = DIR == 0 ? e / NP : e % NT;
+    bool valid;
+    const long long base = line_base(tt, valid);
+    const int node = min(s0 - 4 + pp, n + 3);                     // beyond n+3 nothing is read by a stored result
+    const long long o = base + (long long)node * st;
+    const double r = __ldg(Q + o), mx = __ldg(Q + sv + o), my = __ldg(Q + 2 * sv + o), mz = __ldg(Q + 3 * sv + o);
+    const double E = __ldg(Q + 4 * sv + o);
+    double K[3] = {DIR == 0 ? 1.0 : 0.0, DIR == 1 ? 1.0 : 0.0, DIR == 2 ? 1.0 : 0.0};
+    if constexpr (CURV) {
+      const double J = __ldg(P.detJ + o);
 #pragma unroll
-  for (int c = 0; c < 5; ++c) {
-    const double d = (fl[c] - fr[c]) * sc;                  // step 3, eq. (10)
-    R[c * sv + at] = accumulate ? R[c * sv + at] + d : d;
+      for (int a = 0; a < 3; ++a) K[a] = J * __ldg(P.D[DIR][a] + o);
+    }
+    const double ir = 1.0 / r;
+    const double u = mx * ir, v = my * ir, w = mz * ir;
+    const double p = P.gm1 * (E - 0.5 * (mx * u + my * v + mz * w));
+    const double a = sqrt(P.gamma * p * ir);
+    const int ix = T7::at(pp, tt);
+    pts[0][ix] = r; pts[1][ix] = mx; pts[2][ix] = my; pts[3][ix] = mz; pts[4][ix] = E; pts[5][ix] = p;
+    pts[6][ix] = K[0] * u + K[1] * v + K[2] * w;
+    pts[7][ix] = CURV ? a * sqrt(K[0] * K[0] + K[1] * K[1] + K[2] * K[2]) : a;
+    if constexpr (CURV) { pts[8][ix] = K[0]; pts[9][ix] = K[1]; pts[10][ix] = K[2]; }
+  }
+  __syncthreads();
+
+  // (2) one interface flux per thread: window point m = staged point f + m (m = 3, 4: nodes s0-1+f, s0+f)
+  {
+    // read through a volatile pointer: the staged values are fetched again for every field instead of being kept in
+    // registers across the five fields (the cached form needs more than 255 registers and spills)
+    const volatile double *vp_ = &pts[0][0];
+    auto S = [&](int v, int m) { return vp_[v * (NP * NT) + T7::at(f + m, t)]; };
+    // step 2(a): Roe (or simple) average of the two nodes next to the interface; interface normal from the averaged K
+    double nrm[3] = {DIR == 0 ? 1.0 : 0.0, DIR == 1 ? 1.0 : 0.0, DIR == 2 ? 1.0 : 0.0};
+    if constexpr (CURV) {
+      const double kx = 0.5 * (S(8, 3) + S(8, 4)), ky = 0.5 * (S(9, 3) + S(9, 4)), kz = 0.5 * (S(10, 3) + S(10, 4));
+      const double ik = 1.0 / sqrt(kx * kx + ky * ky + kz * kz);
+      nrm[0] = kx * ik; nrm[1] = ky * ik; nrm[2] = kz * ik;
+    }
+    double u, v, w, H;
+    {
+      const double rL = S(0, 3), rR = S(0, 4);
+      if (P.averaging != 0) {            // U_{i+1/2} = (U_i + U_{i+1})/2
+        const double r = 0.5 * (rL + rR), ir = 1.0 / r;
+        u = 0.5 * (S(1, 3) + S(1, 4)) * ir; v = 0.5 * (S(2, 3) + S(2, 4)) * ir; w = 0.5 * (S(3, 3) + S(3, 4)) * ir;
+        const double E = 0.5 * (S(4, 3) + S(4, 4));
+        const double p = P.gm1 * (E - 0.5 * r * (u * u + v * v + w * w));
+        H = (E + p) * ir;
+      } else {
+        const double sl = sqrt(rL), sr = sqrt(rR), is = 1.0 / (sl + sr);
+        u = (S(1, 3) / sl + S(1, 4) / sr) * is; v = (S(2, 3) / sl + S(2, 4) / sr) * is; w = (S(3, 3) / sl + S(3, 4) / sr) * is;
+        H = ((S(4, 3) + S(5, 3)) / sl + (S(4, 4) + S(5, 4)) / sr) * is;
+      }
+    }
+    const double q2 = u * u + v * v + w * w;
+    const double a = sqrt(P.gm1 * (H - 0.5 * q2));
+    const double th = nrm[0] * u + nrm[1] * v + nrm[2] * w;
+    const double b1 = P.gm1 / (a * a), b2 = 0.5 * b1 * q2, ia = 1.0 / a;
+    const double ut[3] = {u, v, w};
+    // step 2(d): alpha = max over the eight stencil points of |theta|, |theta + c|, |theta - c| (Q10)
+    double al0 = 0.0, alp = 0.0, alm = 0.0;
+#pragma unroll
+    for (int m = 0; m < 8; ++m) {
+      const double thm = S(6, m), cm = S(7, m);
+      al0 = fmax(al0, fabs(thm)); alp = fmax(alp, fabs(thm + cm)); alm = fmax(alm, fabs(thm - cm));
+    }
+    double fh[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+      // step 2(b): row k of L and column k of R for the unit normal nrm (fields 0-2: speed theta; 3, 4: theta +- a)
+      double l[5], rc[5], alpha;
+      if (k < 3) {
+        constexpr int I1[3] = {1, 2, 0}, I2[3] = {2, 0, 1};
+        const int i1 = I1[k], i2 = I2[k];
+        // l_k = n_k (1 - b2, b1 u, -b1) + e_k x n acting on (m - rho u~);  r_k = (n_k, u n_k + (n x e_k), q2/2 n_k + (u x n)_k)
+        l[0] = nrm[k] * (1.0 - b2) - (ut[i1] * nrm[i2] - ut[i2] * nrm[i1]);
+        l[1 + k] = nrm[k] * b1 * ut[k];
+        l[1 + i1] = nrm[k] * b1 * ut[i1] + nrm[i2];
+        l[1 + i2] = nrm[k] * b1 * ut[i2] - nrm[i1];
+        l[4] = -nrm[k] * b1;
+        rc[0] = nrm[k];
+        rc[1 + k] = ut[k] * nrm[k];
+        rc[1 + i1] = ut[i1] * nrm[k] + nrm[i2];
+        rc[1 + i2] = ut[i2] * nrm[k] - nrm[i1];
+        rc[4] = 0.5 * q2 * nrm[k] + ut[i1] * nrm[i2] - ut[i2] * nrm[i1];
+        alpha = al0;
+      } else {
+        const double sg = k == 3 ? 1.0 : -1.0;
+        l[0] = 0.5 * (b2 - sg * th * ia);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { l[1 + c] = 0.5 * (-b1 * ut[c] + sg * nrm[c] * ia); rc[1 + c] = ut[c] + sg * a * nrm[c]; }
+        l[4] = 0.5 * b1;
+        rc[0] = 1.0;
+        rc[4] = H + sg * a * th;
+        alpha = k == 3 ? alp : alm;
+      }
+      // step 2(c), eq. (13): g+- = (l.F +- alpha l.U)/2 with F = theta U + p (0, K, theta)
+      double gp[8], gm[8];
+#pragma unroll
+      for (int m = 0; m < 8; ++m) {
+        const double V = fma(l[0], S(0, m), fma(l[1], S(1, m), fma(l[2], S(2, m), fma(l[3], S(3, m), l[4] * S(4, m)))));
+        const double thm = S(6, m);
+        double lk;
+        if constexpr (CURV) lk = fma(l[1], S(8, m), fma(l[2], S(9, m), fma(l[3], S(10, m), l[4] * thm)));
+        else lk = fma(l[4], thm, l[1 + DIR]);
+        const double G = fma(thm, V, S(5, m) * lk);
+        gp[m] = 0.5 * fma(alpha, V, G);
+        gm[m] = 0.5 * fma(-alpha, V, G);
+      }
+      const double vp[7] = {gp[0], gp[1], gp[2], gp[3], gp[4], gp[5], gp[6]};
+      const double vm[7] = {gm[7], gm[6], gm[5], gm[4], gm[3], gm[2], gm[1]};       // mirror image (Q4)
+      const double gk = weno7z(vp, P.eps) + weno7z(vm, P.eps);                       // step 2(e)
+#pragma unroll
+      for (int c = 0; c < 5; ++c) fh[c] = fma(gk, rc[c], fh[c]);                    // step 2(f)
+    }
+    const int fx = T7::fat(f, t);
+#pragma unroll
+    for (int c = 0; c < 5; ++c) flx[c][fx] = fh[c];
+  }
+  __syncthreads();
+
+  // (3) flux difference of node s0 + f, eq. (10)
+  bool valid;
+  const long long base = line_base(t, valid);
+  const int node = s0 + f;
+  if (valid && f < NS && node < n) {
+    const long long o = base + (long long)node * st;
+    double sc = P.inv_delta[DIR];
+    if constexpr (CURV) sc = 1.0 / __ldg(P.detJ + o);
+    const int f0 = T7::fat(f, t), f1 = T7::fat(f + 1, t);
+#pragma unroll
+    for (int c = 0; c < 5; ++c) {
+      const double d = (flx[c][f0] - flx[c][f1]) * sc;
+      R[c * sv + o] = accumulate ? R[c * sv + o] + d : d;
+    }
   }
 }
 
 template <int DIR>
 cudaError_t launch7(const DevParams &P, const double *Q, double *R, int accumulate, cudaStream_t st) {
-  dim3 grid((P.L.n[0] + 127) / 128, P.L.n[1], P.L.n[2]);
-  if (P.curvilinear) sweep7_kernel<DIR, true><<<grid, 128, 0, st>>>(P, Q, R, accumulate);
-  else sweep7_kernel<DIR, false><<<grid, 128, 0, st>>>(P, Q, R, accumulate);
+  const Layout &L = P.L;
+  auto go = [&](auto curv) {
+    constexpr bool CURV = decltype(curv)::value;
+    using T7 = Tile7<DIR, CURV>;
+    dim3 block, grid;
+    if constexpr (DIR == 0) {
+      block = dim3(T7::NF, T7::NT);
+      grid = dim3((L.n[0] + T7::NS - 1) / T7::NS, (L.n[1] * L.n[2] + T7::NT - 1) / T7::NT, 1);
+    } else {
+      block = dim3(T7::NT, T7::NF);
+      grid = dim3((L.n[0] + T7::NT - 1) / T7::NT, DIR == 1 ? L.n[2] : L.n[1], (L.n[DIR] + T7::NS - 1) / T7::NS);
+    }
+    sweep7_kernel<DIR, CURV><<<grid, block, 0, st>>>(P, Q, R, accumulate);
+  };
+  if (P.curvilinear) go(std::true_type{}); else go(std::false_type{});
   return cudaGetLastError();
 }
 
