@@ -28,6 +28,13 @@ struct osbli_ctx {
   bool pipe_ready;
 };
 
+#ifndef OSBLI_UNI_TILED
+#define OSBLI_UNI_TILED 0      // probe: TENO5 x and y sweeps on uniform grids through the tiled kernel
+#endif
+#ifndef OSBLI_CURV_TILED
+#define OSBLI_CURV_TILED 0     // 1: curvilinear grids use the tiled sweeps of osbli_weno7.cu and the separate stage update
+#endif
+
 namespace {
 
 int make_layout(const osbli_params *p, Layout *L) {
@@ -161,6 +168,11 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
     if (P.scheme == OSBLI_SCHEME_WENOZ7) {                          // side scheme: its own untuned sweeps, no fused update
       if (rk) return OSBLI_EINVAL;
       OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep7(P, d, Q, R, accumulate, st));
+    } else if (OSBLI_UNI_TILED && !P.curvilinear && P.scheme == OSBLI_SCHEME_TENO5 && !(d == last && rk)) {   // probe
+      OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep_tiled(P, d, Q, R, accumulate, st));
+    } else if (OSBLI_CURV_TILED && P.curvilinear) {               // curvilinear grids: the tiled sweeps, no fused update
+      if (rk) return OSBLI_EINVAL;
+      OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep_tiled(P, d, Q, R, accumulate, st));
     } else
       OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep(P, d, Q, R, accumulate, d == last ? rk : nullptr, st));
     accumulate = 1;
@@ -195,7 +207,7 @@ int do_step(osbli_ctx *h, int nstages, double *Q, double *Qtmp, double dt, cudaS
     return OSBLI_OK;
   }
   const bool fuse = (h->P.L.n[1] > 1 || h->P.L.n[2] > 1) && h->P.scheme != OSBLI_SCHEME_CENTRAL4 &&
-                    h->P.scheme != OSBLI_SCHEME_WENOZ7;
+                    h->P.scheme != OSBLI_SCHEME_WENOZ7 && !(OSBLI_CURV_TILED && h->P.curvilinear);
   bool wrap = fuse;                  // every active direction periodic: the fused update fills the halos itself
   for (int d = 0; d < 3; ++d)
     if (h->P.L.n[d] > 1 && !h->P.periodic[d]) wrap = false;

@@ -18,6 +18,8 @@ cudaError_t launch_sweep(const DevParams &P, int dir, const double *Q, double *R
 
 // 7th-order WENO-Z sweeps (scheme 6, osbli_weno7.cu): R (-)= flux difference along `dir`; no fused update
 cudaError_t launch_sweep7(const DevParams &P, int dir, const double *Q, double *R, int accumulate, cudaStream_t st);
+// the same tiled kernel for the 5th/6th-order schemes on curvilinear grids (no fused update)
+cudaError_t launch_sweep_tiled(const DevParams &P, int dir, const double *Q, double *R, int accumulate, cudaStream_t st);
 
 // staged primitive fields u, v, w, T (, mu) on the halo-extended grid, then R += viscous terms (osbli_visc.cu)
 cudaError_t launch_primitives(const DevParams &P, const double *Q, double *prim, cudaStream_t st);

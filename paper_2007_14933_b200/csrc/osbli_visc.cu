@@ -259,8 +259,11 @@ __device__ __forceinline__ void viscous_node(const DevParams &P, const double *_
   dst[0] = rold[0] + r1; dst[sv] = rold[1] + r2; dst[2 * sv] = rold[2] + r3; dst[3 * sv] = rold[3] + r4;
 }
 
+#ifndef OSBLI_GV_MINB
+#define OSBLI_GV_MINB 3
+#endif
 template <bool CURV, bool SUTH>
-__global__ void __launch_bounds__(128, 3)
+__global__ void __launch_bounds__(128, OSBLI_GV_MINB)
 viscous_kernel(const __grid_constant__ DevParams P, const double *__restrict__ prim, const double *__restrict__ grad,
                double *__restrict__ R, int accumulate) {
   const Layout &L = P.L;

@@ -6,6 +6,7 @@
 // 5th/6th-order sweeps (an 8-point window of staged points does not fit the register file next to the rest); dense
 // eigenvectors for a general unit normal (uniform grids: e_d), the stage update is the separate rk_update_kernel.  What
 // it shares with the tuned path is the layout, the boundary fills and the viscous kernels; halo depth 4 (Layout::h).
+#include "osbli_flux.cuh"
 #include "osbli_kernels.h"
 
 #include <type_traits>
@@ -64,9 +65,11 @@ __device__ __forceinline__ double weno7z(const double (&v)[7], double eps) {
 // thermodynamics is computed (NS+8)/NS times and every flux (NS+1)/NS times.
 //   y, z sweeps: threadIdx.x = x lane (coalesced rows), threadIdx.y = f;  NS = 8 (6 on curvilinear grids: 3 more
 //   staged doubles per point);   x sweep: threadIdx.x = f (32 interfaces, NS = 31 nodes), threadIdx.y = line of 8.
-template <int DIR, bool CURV> struct Tile7 {
-  static constexpr int NS = DIR == 0 ? 31 : (CURV ? 6 : 8);      // nodes per block along the sweep
-  static constexpr int NF = NS + 1, NP = NS + 8;                  // interfaces, staged points (s0-4 .. s0+NS+3)
+// W = 8: scheme 6 (WENO-Z7).  W = 6: the 5th/6th-order schemes through the same kernel (OSBLI_CURV_TILED, curvilinear grids).
+template <int DIR, bool CURV, int W> struct Tile7 {
+  static constexpr int H = W / 2;                                 // window point H-1 = node i, H = node i+1 of interface i+1/2
+  static constexpr int NS = DIR == 0 ? 31 : (CURV ? (W == 8 ? 6 : 7) : 8);      // nodes per block along the sweep
+  static constexpr int NF = NS + 1, NP = NS + W;                  // interfaces, staged points (s0-H .. s0+NS+H-1)
   static constexpr int NT = DIR == 0 ? 8 : 32;                    // lines per block
   static constexpr int NV = CURV ? 11 : 8;                        // staged doubles per point
   static constexpr int NTHREADS = NF * NT;
@@ -75,11 +78,13 @@ template <int DIR, bool CURV> struct Tile7 {
   static __device__ __forceinline__ int fat(int f, int t) { return DIR == 0 ? t * NF + f : f * NT + t; }
 };
 
-template <int DIR, bool CURV>
-__global__ void __launch_bounds__((Tile7<DIR, CURV>::NTHREADS), 2)
+template <int DIR, bool CURV, int SCHEME>
+__global__ void __launch_bounds__((Tile7<DIR, CURV, SCHEME == 6 ? 8 : 6>::NTHREADS), 2)
 sweep7_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q, double *__restrict__ R, int accumulate) {
-  using T7 = Tile7<DIR, CURV>;
-  constexpr int NS = T7::NS, NF = T7::NF, NP = T7::NP, NT = T7::NT, NV = T7::NV;
+  constexpr int W = SCHEME == 6 ? 8 : 6;
+  using T7 = Tile7<DIR, CURV, W>;
+  constexpr int NS = T7::NS, NF = T7::NF, NP = T7::NP, NT = T7::NT, NV = T7::NV, HL = T7::H - 1, HR = T7::H;
+  const RecPar rp = make_recpar(P);
   __shared__ double pts[NV][NP * NT];
   __shared__ double flx[5][NF * NT];
   const Layout &L = P.L;
@@ -111,7 +116,7 @@ sweep7_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q,
     const int pp = DIR == 0 ? e % NP : e / NT, tt = DIR == 0 ? e / NP : e % NT;
     bool valid;
     const long long base = line_base(tt, valid);
-    const int node = min(s0 - 4 + pp, n + 3);                     // beyond n+3 nothing is read by a stored result
+    const int node = min(s0 - T7::H + pp, n + T7::H - 1);         // beyond n+H-1 nothing is read by a stored result
     const long long o = base + (long long)node * st;
     const double r = __ldg(Q + o), mx = __ldg(Q + sv + o), my = __ldg(Q + 2 * sv + o), mz = __ldg(Q + 3 * sv + o);
     const double E = __ldg(Q + 4 * sv + o);
@@ -133,7 +138,7 @@ sweep7_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q,
   }
   __syncthreads();
 
-  // (2) one interface flux per thread: window point m = staged point f + m (m = 3, 4: nodes s0-1+f, s0+f)
+  // (2) one interface flux per thread: window point m = staged point f + m (m = HL, HR: nodes s0-1+f, s0+f)
   {
     // read through a volatile pointer: the staged values are fetched again for every field instead of being kept in
     // registers across the five fields (the cached form needs more than 255 registers and spills)
@@ -142,23 +147,23 @@ sweep7_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q,
     // step 2(a): Roe (or simple) average of the two nodes next to the interface; interface normal from the averaged K
     double nrm[3] = {DIR == 0 ? 1.0 : 0.0, DIR == 1 ? 1.0 : 0.0, DIR == 2 ? 1.0 : 0.0};
     if constexpr (CURV) {
-      const double kx = 0.5 * (S(8, 3) + S(8, 4)), ky = 0.5 * (S(9, 3) + S(9, 4)), kz = 0.5 * (S(10, 3) + S(10, 4));
+      const double kx = 0.5 * (S(8, HL) + S(8, HR)), ky = 0.5 * (S(9, HL) + S(9, HR)), kz = 0.5 * (S(10, HL) + S(10, HR));
       const double ik = 1.0 / sqrt(kx * kx + ky * ky + kz * kz);
       nrm[0] = kx * ik; nrm[1] = ky * ik; nrm[2] = kz * ik;
     }
     double u, v, w, H;
     {
-      const double rL = S(0, 3), rR = S(0, 4);
+      const double rL = S(0, HL), rR = S(0, HR);
       if (P.averaging != 0) {            // U_{i+1/2} = (U_i + U_{i+1})/2
         const double r = 0.5 * (rL + rR), ir = 1.0 / r;
-        u = 0.5 * (S(1, 3) + S(1, 4)) * ir; v = 0.5 * (S(2, 3) + S(2, 4)) * ir; w = 0.5 * (S(3, 3) + S(3, 4)) * ir;
-        const double E = 0.5 * (S(4, 3) + S(4, 4));
+        u = 0.5 * (S(1, HL) + S(1, HR)) * ir; v = 0.5 * (S(2, HL) + S(2, HR)) * ir; w = 0.5 * (S(3, HL) + S(3, HR)) * ir;
+        const double E = 0.5 * (S(4, HL) + S(4, HR));
         const double p = P.gm1 * (E - 0.5 * r * (u * u + v * v + w * w));
         H = (E + p) * ir;
       } else {
         const double sl = sqrt(rL), sr = sqrt(rR), is = 1.0 / (sl + sr);
-        u = (S(1, 3) / sl + S(1, 4) / sr) * is; v = (S(2, 3) / sl + S(2, 4) / sr) * is; w = (S(3, 3) / sl + S(3, 4) / sr) * is;
-        H = ((S(4, 3) + S(5, 3)) / sl + (S(4, 4) + S(5, 4)) / sr) * is;
+        u = (S(1, HL) / sl + S(1, HR) / sr) * is; v = (S(2, HL) / sl + S(2, HR) / sr) * is; w = (S(3, HL) / sl + S(3, HR) / sr) * is;
+        H = ((S(4, HL) + S(5, HL)) / sl + (S(4, HR) + S(5, HR)) / sr) * is;
       }
     }
     const double q2 = u * u + v * v + w * w;
@@ -169,7 +174,7 @@ sweep7_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q,
     // step 2(d): alpha = max over the eight stencil points of |theta|, |theta + c|, |theta - c| (Q10)
     double al0 = 0.0, alp = 0.0, alm = 0.0;
 #pragma unroll
-    for (int m = 0; m < 8; ++m) {
+    for (int m = 0; m < W; ++m) {
       const double thm = S(6, m), cm = S(7, m);
       al0 = fmax(al0, fabs(thm)); alp = fmax(alp, fabs(thm + cm)); alm = fmax(alm, fabs(thm - cm));
     }
@@ -204,27 +209,32 @@ sweep7_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q,
         alpha = k == 3 ? alp : alm;
       }
       // step 2(c), eq. (13): g+- = (l.F +- alpha l.U)/2 with F = theta U + p (0, K, theta)
-      double gp[8], gm[8];
+      double gp[W], gm[W];
 #pragma unroll
-      for (int m = 0; m < 8; ++m) {
+      for (int m = 0; m < W; ++m) {
         const double V = fma(l[0], S(0, m), fma(l[1], S(1, m), fma(l[2], S(2, m), fma(l[3], S(3, m), l[4] * S(4, m)))));
         const double thm = S(6, m);
         double lk;
         if constexpr (CURV) lk = fma(l[1], S(8, m), fma(l[2], S(9, m), fma(l[3], S(10, m), l[4] * thm)));
         else lk = fma(l[4], thm, l[1 + DIR]);
         const double G = fma(thm, V, S(5, m) * lk);
-        gp[m] = 0.5 * fma(alpha, V, G);
-        gm[m] = 0.5 * fma(-alpha, V, G);
+        gp[m] = fma(alpha, V, G);                            // twice the split fluxes
+        gm[m] = fma(-alpha, V, G);
       }
-      const double vp[7] = {gp[0], gp[1], gp[2], gp[3], gp[4], gp[5], gp[6]};
-      const double vm[7] = {gm[7], gm[6], gm[5], gm[4], gm[3], gm[2], gm[1]};       // mirror image (Q4)
-      const double gk = weno7z(vp, P.eps) + weno7z(vm, P.eps);                       // step 2(e)
+      double gk;                                             // twice (g^+ + g^-), step 2(e)
+      if constexpr (W == 8) {
+        const double vp[7] = {0.5 * gp[0], 0.5 * gp[1], 0.5 * gp[2], 0.5 * gp[3], 0.5 * gp[4], 0.5 * gp[5], 0.5 * gp[6]};
+        const double vm[7] = {0.5 * gm[7], 0.5 * gm[6], 0.5 * gm[5], 0.5 * gm[4], 0.5 * gm[3], 0.5 * gm[2], 0.5 * gm[1]};   // mirror image (Q4)
+        gk = 2.0 * (weno7z(vp, P.eps) + weno7z(vm, P.eps));
+      } else {
+        gk = reconstruct_pair<SCHEME>(gp, gm, rp);           // osbli_flux.cuh: data and result carry the factor 2
+      }
 #pragma unroll
       for (int c = 0; c < 5; ++c) fh[c] = fma(gk, rc[c], fh[c]);                    // step 2(f)
     }
     const int fx = T7::fat(f, t);
 #pragma unroll
-    for (int c = 0; c < 5; ++c) flx[c][fx] = fh[c];
+    for (int c = 0; c < 5; ++c) flx[c][fx] = 0.5 * fh[c];          // the 1/2 of eq. (13)
   }
   __syncthreads();
 
@@ -245,12 +255,12 @@ sweep7_kernel(const __grid_constant__ DevParams P, const double *__restrict__ Q,
   }
 }
 
-template <int DIR>
+template <int DIR, int SCHEME>
 cudaError_t launch7(const DevParams &P, const double *Q, double *R, int accumulate, cudaStream_t st) {
   const Layout &L = P.L;
   auto go = [&](auto curv) {
     constexpr bool CURV = decltype(curv)::value;
-    using T7 = Tile7<DIR, CURV>;
+    using T7 = Tile7<DIR, CURV, SCHEME == 6 ? 8 : 6>;
     dim3 block, grid;
     if constexpr (DIR == 0) {
       block = dim3(T7::NF, T7::NT);
@@ -259,18 +269,42 @@ cudaError_t launch7(const DevParams &P, const double *Q, double *R, int accumula
       block = dim3(T7::NT, T7::NF);
       grid = dim3((L.n[0] + T7::NT - 1) / T7::NT, DIR == 1 ? L.n[2] : L.n[1], (L.n[DIR] + T7::NS - 1) / T7::NS);
     }
-    sweep7_kernel<DIR, CURV><<<grid, block, 0, st>>>(P, Q, R, accumulate);
+    sweep7_kernel<DIR, CURV, SCHEME><<<grid, block, 0, st>>>(P, Q, R, accumulate);
   };
-  if (P.curvilinear) go(std::true_type{}); else go(std::false_type{});
+  if constexpr (SCHEME == 6) {
+    if (P.curvilinear) go(std::true_type{}); else go(std::false_type{});
+  } else {
+    if (P.curvilinear) go(std::true_type{});
+    else if constexpr (SCHEME == 1) go(std::false_type{});   // probe (OSBLI_UNI_TILED): TENO5 on uniform grids
+  }
   return cudaGetLastError();
+}
+
+template <int SCHEME>
+cudaError_t launch7_dir(const DevParams &P, int dir, const double *Q, double *R, int accumulate, cudaStream_t st) {
+  if (dir == 0) return launch7<0, SCHEME>(P, Q, R, accumulate, st);
+  if (dir == 1) return launch7<1, SCHEME>(P, Q, R, accumulate, st);
+  return launch7<2, SCHEME>(P, Q, R, accumulate, st);
 }
 
 }  // namespace
 
 cudaError_t launch_sweep7(const DevParams &P, int dir, const double *Q, double *R, int accumulate, cudaStream_t st) {
-  if (dir == 0) return launch7<0>(P, Q, R, accumulate, st);
-  if (dir == 1) return launch7<1>(P, Q, R, accumulate, st);
-  return launch7<2>(P, Q, R, accumulate, st);
+  return launch7_dir<6>(P, dir, Q, R, accumulate, st);
+}
+
+// The 5th/6th-order schemes on curvilinear grids through the tiled kernel (one flux per thread, points in shared
+// memory, no fused stage update): scheme 0 WENO-Z5, 1 TENO5, 2 TENO6, 3 WENO-JS5, 5 WENO-Z3.
+cudaError_t launch_sweep_tiled(const DevParams &P, int dir, const double *Q, double *R, int accumulate, cudaStream_t st) {
+  if (!P.curvilinear && P.scheme != 1) return cudaErrorInvalidValue;
+  switch (P.scheme) {
+    case 0: return launch7_dir<0>(P, dir, Q, R, accumulate, st);
+    case 1: return launch7_dir<1>(P, dir, Q, R, accumulate, st);
+    case 2: return launch7_dir<2>(P, dir, Q, R, accumulate, st);
+    case 3: return launch7_dir<3>(P, dir, Q, R, accumulate, st);
+    case 5: return launch7_dir<5>(P, dir, Q, R, accumulate, st);
+    default: return cudaErrorInvalidValue;
+  }
 }
 
 }  // namespace osbli
