@@ -28,12 +28,9 @@ struct osbli_ctx {
   bool pipe_ready;
 };
 
-#ifndef OSBLI_UNI_TILED
-#define OSBLI_UNI_TILED 0      // probe: TENO5 x and y sweeps on uniform grids through the tiled kernel
-#endif
-#ifndef OSBLI_CURV_TILED
-#define OSBLI_CURV_TILED 0     // 1: curvilinear grids use the tiled sweeps of osbli_weno7.cu and the separate stage update
-#endif
+#ifndef OSBLI_CURV_TILED_X
+#define OSBLI_CURV_TILED_X 1   // curvilinear grids: the x sweep runs on the tiled kernel of osbli_weno7.cu (config 4: 0.180 -> 0.149 ms;
+#endif                        // the y and z sweeps lose there: 0.134 -> 0.178, 0.139 -> 0.301 with 8 nodes along z)
 
 namespace {
 
@@ -168,10 +165,10 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
     if (P.scheme == OSBLI_SCHEME_WENOZ7) {                          // side scheme: its own untuned sweeps, no fused update
       if (rk) return OSBLI_EINVAL;
       OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep7(P, d, Q, R, accumulate, st));
-    } else if (OSBLI_UNI_TILED && !P.curvilinear && P.scheme == OSBLI_SCHEME_TENO5 && !(d == last && rk)) {   // probe
-      OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep_tiled(P, d, Q, R, accumulate, st));
-    } else if (OSBLI_CURV_TILED && P.curvilinear) {               // curvilinear grids: the tiled sweeps, no fused update
-      if (rk) return OSBLI_EINVAL;
+    } else if (OSBLI_CURV_TILED_X && P.curvilinear && d == 0 && !(d == last && rk) &&
+               (long long)((P.L.n[1] * P.L.n[2] + 31) / 32) * ((P.L.n[0] + 63) / 64) < 148LL * 8) {
+      // curvilinear x sweep on grids whose 64-node line segments do not fill the chip's warp slots (config 4): the tiled
+      // kernel, one thread per interface, instead of the march with 16-node segments
       OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep_tiled(P, d, Q, R, accumulate, st));
     } else
       OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X + d, st, launch_sweep(P, d, Q, R, accumulate, d == last ? rk : nullptr, st));
@@ -207,7 +204,7 @@ int do_step(osbli_ctx *h, int nstages, double *Q, double *Qtmp, double dt, cudaS
     return OSBLI_OK;
   }
   const bool fuse = (h->P.L.n[1] > 1 || h->P.L.n[2] > 1) && h->P.scheme != OSBLI_SCHEME_CENTRAL4 &&
-                    h->P.scheme != OSBLI_SCHEME_WENOZ7 && !(OSBLI_CURV_TILED && h->P.curvilinear);
+                    h->P.scheme != OSBLI_SCHEME_WENOZ7;
   bool wrap = fuse;                  // every active direction periodic: the fused update fills the halos itself
   for (int d = 0; d < 3; ++d)
     if (h->P.L.n[d] > 1 && !h->P.periodic[d]) wrap = false;

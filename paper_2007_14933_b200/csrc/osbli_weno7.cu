@@ -274,8 +274,7 @@ cudaError_t launch7(const DevParams &P, const double *Q, double *R, int accumula
   if constexpr (SCHEME == 6) {
     if (P.curvilinear) go(std::true_type{}); else go(std::false_type{});
   } else {
-    if (P.curvilinear) go(std::true_type{});
-    else if constexpr (SCHEME == 1) go(std::false_type{});   // probe (OSBLI_UNI_TILED): TENO5 on uniform grids
+    go(std::true_type{});                                    // the 5th/6th-order schemes come here on curvilinear grids only
   }
   return cudaGetLastError();
 }
@@ -296,7 +295,7 @@ cudaError_t launch_sweep7(const DevParams &P, int dir, const double *Q, double *
 // The 5th/6th-order schemes on curvilinear grids through the tiled kernel (one flux per thread, points in shared
 // memory, no fused stage update): scheme 0 WENO-Z5, 1 TENO5, 2 TENO6, 3 WENO-JS5, 5 WENO-Z3.
 cudaError_t launch_sweep_tiled(const DevParams &P, int dir, const double *Q, double *R, int accumulate, cudaStream_t st) {
-  if (!P.curvilinear && P.scheme != 1) return cudaErrorInvalidValue;
+  if (!P.curvilinear) return cudaErrorInvalidValue;
   switch (P.scheme) {
     case 0: return launch7_dir<0>(P, dir, Q, R, accumulate, st);
     case 1: return launch7_dir<1>(P, dir, Q, R, accumulate, st);
