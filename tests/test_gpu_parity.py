@@ -365,11 +365,11 @@ def test_advance_host_batch_pipeline_matches_serial():
 
 
 # ------------------------------------------------- full size, bench launch configuration ----
-def sampled_full_size(name, n, nsamples, presteps):
+def sampled_full_size(name, n, nsamples, presteps, scheme=W.TENO5):
     """At BASELINE.json's full sizes the oracle is evaluated one node at a time on sampled nodes
     (oracle_rhs_points) of the state the GPU produced after `presteps` steps."""
     torch = _torch()
-    case = W.tgv(n)
+    case = W.tgv(n, scheme=scheme)
     sol = parity.make_solver(case)
     Q = sol.to_padded(case.Q0)
     Qtmp = sol.empty_state()
@@ -405,6 +405,12 @@ def sampled_full_size(name, n, nsamples, presteps):
 
 def test_full_size_tgv256_config3_sampled():
     sampled_full_size("tgv256_sampled", 256, 3000, presteps=2)
+
+
+def test_full_size_tgv256_wenoz7_sampled():
+    """The tiled WENO-Z7 kernel in the launch configuration bench.py --scheme wenoz7 times (256^3: 9 x 8 x 32 blocks of
+    32 x 9 threads along y and z, 31-node tiles along x with a ragged last tile)."""
+    sampled_full_size("tgv256_wenoz7_sampled", 256, 1500, presteps=1, scheme=W.WENOZ7)
 
 
 def test_full_size_tgv256_config3_state_3_steps():
