@@ -24,7 +24,7 @@ from paper_2007_14933_b200 import workloads as W                 # noqa: E402
 
 def periodic_box(n, scheme=W.TENO5, visc=W.VISC_CONST):
     c = W.tgv(8, scheme=scheme, visc=visc)
-    i, j, k = W.padded_index_grids(n)
+    i, j, k = W.padded_index_grids(n, scheme)
     x, y, z = 2 * np.pi * i / n[0], 2 * np.pi * j / n[1], 2 * np.pi * k / n[2]
     g, M = 1.4, 0.4
     u = np.sin(x) * np.cos(y) * np.cos(z)
@@ -74,6 +74,9 @@ def main():
     ssp = W.tgv(16)
     ssp.rk3_form, ssp.averaging = W.RK3_SSP, W.AVG_SIMPLE
     run("tgv16_ssp_simple_avg", ssp, 1)
+    run("pbox_37x21x13_wenoz7 (halo 4, tiled sweeps)", periodic_box((37, 21, 13), scheme=W.WENOZ7), 1)
+    wb7 = W.wavy_box(n=(40, 21, 9), scheme=W.WENOZ7)
+    run("wavy_box_wenoz7", wb7, 1, metrics=W.approximate_metrics(wb7))
     print("sanitizer cases done")
 
 

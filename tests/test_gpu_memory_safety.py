@@ -25,7 +25,7 @@ GUARD = 1 << 16           # doubles on either side of every carved buffer (512 K
 
 
 NAMES = ("tgv32_teno5", "pbox_5x7x6", "pbox_70x37x35_teno6", "pbox2d_40x33", "pbox_mixed_bc", "sod", "tgv16_central4",
-         "wavy_box", "channel3d", "tgv16_ssp_simple")
+         "wavy_box", "channel3d", "tgv16_ssp_simple", "pbox_37x21x13_wenoz7", "wavy_box_wenoz7", "sod_wenoz7")
 
 
 def _case(name):
@@ -43,6 +43,9 @@ def _case(name):
             "sod": lambda: (W.sod(), 20),
             "tgv16_central4": lambda: (W.tgv(16, scheme=W.CENTRAL4), 2),
             "wavy_box": lambda: (W.wavy_box(n=(40, 21, 9)), 2),
+            "pbox_37x21x13_wenoz7": lambda: (_periodic_box((37, 21, 13), scheme=W.WENOZ7), 2),    # halo 4, tiled sweeps, ragged tiles
+            "wavy_box_wenoz7": lambda: (W.wavy_box(n=(40, 21, 9), scheme=W.WENOZ7), 2),
+            "sod_wenoz7": lambda: (W.sod(scheme=W.WENOZ7), 20),
             "channel3d": lambda: (W.channel(n=(24, 33, 6), noise=1e-3, scheme=W.TENO5), 2)}[name]()
 
 
