@@ -118,6 +118,10 @@ int osbli_workspace_bytes(const osbli_params *p, size_t *out);
  * paired, gamma <= 1, eps < 1e-18, missing dirichlet / metrics pointers), OSBLI_EUNSUPPORTED
  * (nx == 1: x is the contiguous direction and must be active; boundary types of an inactive
  * direction are ignored), OSBLI_ECUDA (no sm_100 device / runtime failure). */
+/* A handle whose configuration takes the general viscous path (non-periodic, curvilinear or Sutherland) also owns one
+ * CUDA stream and two events: osbli_rhs / osbli_rk3_step form the staged primitive fields and their first differences
+ * on it, next to the first sweeps, forked from and joined back into the caller's stream by events (nothing is
+ * synchronised on the host; to the caller the work stays ordered on the stream it passed). */
 int osbli_init(const osbli_params *p, void *d_workspace, size_t workspace_bytes, osbli_handle *out);
 
 /* Fill the halos (depth layout.halo) (and, for DIRICHLET / WALL, the boundary plane) of device state Q in

@@ -26,8 +26,16 @@ struct osbli_ctx {
   cudaStream_t s_in, s_out;            // copy streams of osbli_advance_host_batch (created on first use)
   cudaEvent_t ev_h2d[3], ev_cmp[3], ev_d2h[3];
   bool pipe_ready;
+  // general viscous path: the staged primitives and their first differences depend on Q only and are formed on a side
+  // stream next to the first sweeps (created by osbli_init; absent in osbli_rk3_step_static, which creates nothing)
+  cudaStream_t s_side;
+  cudaEvent_t ev_fork, ev_join;
+  bool side_ready;
 };
 
+#ifndef OSBLI_SIDE_STREAM
+#define OSBLI_SIDE_STREAM 1    // general viscous path: primitives + first differences on a side stream next to the first sweeps
+#endif
 #ifndef OSBLI_CURV_TILED_X
 #define OSBLI_CURV_TILED_X 1   // curvilinear grids: the x sweep runs on the tiled kernel of osbli_weno7.cu (config 4: 0.180 -> 0.149 ms;
 #endif                        // the y and z sweeps lose there: 0.134 -> 0.178, 0.139 -> 0.301 with 8 nodes along z)
@@ -136,7 +144,20 @@ int do_bc(osbli_ctx *h, double *Q, cudaStream_t st) {
 int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStream_t st) {
   const DevParams &P = h->P;
   const bool fast_visc = viscous_fast_path(P);
-  if (P.visc != OSBLI_VISC_NONE && !fast_visc) OSBLI_LAUNCH(h, OSBLI_K_PRIM, st, launch_primitives(P, Q, h->prim, st));
+  const bool general_visc = P.visc != OSBLI_VISC_NONE && !fast_visc;
+  int last = 0;
+  for (int d = 0; d < 3; ++d)
+    if (P.L.n[d] > 1) last = d;
+  // fork: primitives and first differences on the side stream while the first sweeps run (2-D / 3-D sweeps path only)
+  const bool fork = OSBLI_SIDE_STREAM && general_visc && h->side_ready && last > 0 && P.scheme != OSBLI_SCHEME_CENTRAL4;
+  if (fork) {
+    if (cudaEventRecord(h->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(h->s_side, h->ev_fork, 0) != cudaSuccess) return OSBLI_ECUDA;
+    OSBLI_LAUNCH(h, OSBLI_K_PRIM, h->s_side, launch_primitives(P, Q, h->prim, h->s_side));
+    OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, h->s_side, launch_gradients(P, h->prim, h->s_side));
+    if (cudaEventRecord(h->ev_join, h->s_side) != cudaSuccess) return OSBLI_ECUDA;
+  } else if (general_visc) {
+    OSBLI_LAUNCH(h, OSBLI_K_PRIM, st, launch_primitives(P, Q, h->prim, st));
+  }
   if (P.scheme == OSBLI_SCHEME_CENTRAL4) {                            // no sweeps: central convective terms, then the rest
     if (rk) return OSBLI_EINVAL;
     OSBLI_LAUNCH(h, OSBLI_K_SWEEP_X, st, launch_central(P, Q, R, st));
@@ -148,15 +169,15 @@ int do_rhs(osbli_ctx *h, const double *Q, double *R, const RkArgs *rk, cudaStrea
     if (P.has_force) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_force(P, Q, R, st));
     return OSBLI_OK;
   }
-  int last = 0;
-  for (int d = 0; d < 3; ++d)
-    if (P.L.n[d] > 1) last = d;
   int accumulate = 0;
   for (int d = 0; d < 3; ++d) {
     if (P.L.n[d] <= 1) continue;
     if (d == last && last > 0) {                                    // viscous terms go in front of the last sweep
       if (fast_visc) OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous_fast(P, Q, R, &h->tmaps, st));
-      else if (P.visc != OSBLI_VISC_NONE) {
+      else if (fork) {                                              // join: the first differences are there
+        if (cudaStreamWaitEvent(st, h->ev_join, 0) != cudaSuccess) return OSBLI_ECUDA;
+        OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous_assemble(P, h->prim, R, accumulate, st));
+      } else if (P.visc != OSBLI_VISC_NONE) {
         OSBLI_LAUNCH(h, OSBLI_K_VISCOUS, st, launch_viscous(P, Q, h->prim, R, accumulate, st));
         ++h->launches;                                              // launch_viscous = gradients_kernel + viscous_kernel
       }
@@ -315,6 +336,13 @@ int osbli_init(const osbli_params *p, void *d_workspace, size_t workspace_bytes,
   fill_ctx(p, d_workspace, h);
   h->prof = new (std::nothrow) std::vector<ProfiledLaunch>();
   if (!h->prof) { delete h; return OSBLI_EINVAL; }
+  if (nprim(p) > 0) {                                              // side stream of the general viscous path
+    if (cudaStreamCreateWithFlags(&h->s_side, cudaStreamNonBlocking) == cudaSuccess &&
+        cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
+        cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) == cudaSuccess)
+      h->side_ready = true;
+    else { delete h->prof; delete h; return OSBLI_ECUDA; }
+  }
   *out = h;
   return OSBLI_OK;
 }
@@ -462,6 +490,11 @@ int osbli_destroy(osbli_handle h) {
   if (h->prof) {
     for (ProfiledLaunch &pl : *h->prof) { cudaEventDestroy(pl.t0); cudaEventDestroy(pl.t1); }
     delete h->prof;
+  }
+  if (h->side_ready) {
+    cudaStreamDestroy(h->s_side);
+    cudaEventDestroy(h->ev_fork);
+    cudaEventDestroy(h->ev_join);
   }
   if (h->pipe_ready) {
     cudaStreamDestroy(h->s_in);

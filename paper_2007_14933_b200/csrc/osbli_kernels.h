@@ -24,6 +24,9 @@ cudaError_t launch_sweep_tiled(const DevParams &P, int dir, const double *Q, dou
 // staged primitive fields u, v, w, T (, mu) on the halo-extended grid, then R += viscous terms (osbli_visc.cu)
 cudaError_t launch_primitives(const DevParams &P, const double *Q, double *prim, cudaStream_t st);
 cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *prim, double *R, int accumulate, cudaStream_t st);
+// its two kernels on their own: the first differences of the staged fields (depend on Q only), then the assembly (R +=)
+cudaError_t launch_gradients(const DevParams &P, const double *prim, cudaStream_t st);
+cudaError_t launch_viscous_assemble(const DevParams &P, const double *prim, double *R, int accumulate, cudaStream_t st);
 
 // fused fast path (uniform grid, mu = 1, three periodic directions): reads Q directly, R += viscous terms
 bool viscous_fast_path(const DevParams &P);

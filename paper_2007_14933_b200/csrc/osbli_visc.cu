@@ -337,23 +337,28 @@ cudaError_t launch_primitives(const DevParams &P, const double *Q, double *prim,
   return cudaGetLastError();
 }
 
-cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *prim, double *R, int accumulate,
-                           cudaStream_t st) {
-  (void)Q;
+// stored first differences live behind the staged primitive fields in the workspace (osbli_workspace_bytes)
+static double *grad_fields(const DevParams &P, const double *prim) {
+  return const_cast<double *>(prim) + (long long)(P.visc == 2 ? 5 : 4) * P.L.sv;
+}
+
+cudaError_t launch_gradients(const DevParams &P, const double *prim, cudaStream_t st) {
   const Layout &L = P.L;
   const bool curv = P.curvilinear != 0, suth = P.visc == 2;
-  // stored first differences live behind the staged primitive fields in the workspace (osbli_workspace_bytes)
-  double *grad = const_cast<double *>(prim) + (long long)(suth ? 5 : 4) * L.sv;
-  {
-    int ext[3];
-    for (int d = 0; d < 3; ++d) ext[d] = (L.n[d] > 1 && P.periodic[d]) ? 2 : 0;
-    const int NX = L.n[0] + 2 * ext[0];
-    dim3 grid((NX + 127) / 128, L.n[1] + 2 * ext[1], L.n[2] + 2 * ext[2]);
-    if (suth) gradients_kernel<5><<<grid, 128, 0, st>>>(P, prim, grad, curv ? 1 : 0);
-    else gradients_kernel<4><<<grid, 128, 0, st>>>(P, prim, grad, curv ? 1 : 0);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-  }
+  double *grad = grad_fields(P, prim);
+  int ext[3];
+  for (int d = 0; d < 3; ++d) ext[d] = (L.n[d] > 1 && P.periodic[d]) ? 2 : 0;
+  const int NX = L.n[0] + 2 * ext[0];
+  dim3 grid((NX + 127) / 128, L.n[1] + 2 * ext[1], L.n[2] + 2 * ext[2]);
+  if (suth) gradients_kernel<5><<<grid, 128, 0, st>>>(P, prim, grad, curv ? 1 : 0);
+  else gradients_kernel<4><<<grid, 128, 0, st>>>(P, prim, grad, curv ? 1 : 0);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_viscous_assemble(const DevParams &P, const double *prim, double *R, int accumulate, cudaStream_t st) {
+  const Layout &L = P.L;
+  const bool curv = P.curvilinear != 0, suth = P.visc == 2;
+  const double *grad = grad_fields(P, prim);
   const int bx = L.n[0] >= 128 ? 128 : 64;
   dim3 grid((L.n[0] + bx - 1) / bx, L.n[1], L.n[2]);
   if (curv && suth) viscous_kernel<true, true><<<grid, bx, 0, st>>>(P, prim, grad, R, accumulate);
@@ -361,6 +366,14 @@ cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *pr
   else if (suth) viscous_kernel<false, true><<<grid, bx, 0, st>>>(P, prim, grad, R, accumulate);
   else viscous_kernel<false, false><<<grid, bx, 0, st>>>(P, prim, grad, R, accumulate);
   return cudaGetLastError();
+}
+
+cudaError_t launch_viscous(const DevParams &P, const double *Q, const double *prim, double *R, int accumulate,
+                           cudaStream_t st) {
+  (void)Q;
+  cudaError_t e = launch_gradients(P, prim, st);
+  if (e != cudaSuccess) return e;
+  return launch_viscous_assemble(P, prim, R, accumulate, st);
 }
 
 // =============================================================================================
