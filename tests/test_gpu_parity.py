@@ -365,11 +365,13 @@ def test_advance_host_batch_pipeline_matches_serial():
 
 
 # ------------------------------------------------- full size, bench launch configuration ----
-def sampled_full_size(name, n, nsamples, presteps, scheme=W.TENO5):
+def sampled_full_size(name, n, nsamples, presteps, scheme=W.TENO5, perturb=0.0):
     """At BASELINE.json's full sizes the oracle is evaluated one node at a time on sampled nodes
     (oracle_rhs_points) of the state the GPU produced after `presteps` steps."""
     torch = _torch()
     case = W.tgv(n, scheme=scheme)
+    if perturb:
+        case.Q0 = W.perturb(case, seed=5, amp=perturb)          # the seed bench.py uses
     sol = parity.make_solver(case)
     Q = sol.to_padded(case.Q0)
     Qtmp = sol.empty_state()
@@ -405,6 +407,12 @@ def sampled_full_size(name, n, nsamples, presteps, scheme=W.TENO5):
 
 def test_full_size_tgv256_config3_sampled():
     sampled_full_size("tgv256_sampled", 256, 3000, presteps=2)
+
+
+def test_full_size_tgv256_perturbed_sampled():
+    """The state of `bench.py --perturb 0.05` (most reconstructions take the divergent full TENO5 evaluation) in the
+    launch configuration of the headline run."""
+    sampled_full_size("tgv256_perturbed_sampled", 256, 1500, presteps=1, perturb=0.05)
 
 
 def test_full_size_tgv256_wenoz7_sampled():
