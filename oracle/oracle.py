@@ -195,6 +195,9 @@ def metrics_from_coords(coords, n, periodic, delta=(1.0, 1.0, 1.0), nthreads=Non
     halo-filled fields in oracle layout.  `scheme` only selects the halo depth (4 for WENO-7Z).
     """
     coords = np.ascontiguousarray(coords, dtype=np.float64)
+    hd = 4 if int(scheme) == WENOZ7 else 3
+    want = tuple(int(v) + (2 * hd if int(v) > 1 else 0) for v in reversed(tuple(n)))
+    assert coords.shape == (3,) + want, (coords.shape, want, "coords must carry the halo depth of `scheme`")
     p = _Params()
     p.scheme = int(scheme)
     p.n[:] = [int(v) for v in n]

@@ -18,7 +18,7 @@ def make(case, **over):
     kw.update(over)
     metrics = None
     if case.coords is not None:
-        metrics = O.metrics_from_coords(case.coords, case.n, case.periodic, delta=case.delta)
+        metrics = O.metrics_from_coords(case.coords, case.n, case.periodic, delta=case.delta, scheme=kw["scheme"])
     return O.Oracle(metrics=metrics, **kw)
 
 
